@@ -1,0 +1,151 @@
+"""ctypes front end of the CPU oracle ``oracle/lra_ref.c``.  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, ``__graft_entry__.smoke()`` and bench.py's ``cpu_baseline`` / ``--impl reference`` legs
+import this module; nothing under ``paper_2508_17187_b200/`` does.  The functions marshal numpy
+arrays into the C calls and do no arithmetic of their own.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "liblra_ref.so")
+_SRC = os.path.join(_HERE, "lra_ref.c")
+
+SORT_TILE, SORT_TILE_CF = 0, 1
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2 -ffp-contract=off -fopenmp: no FMA contraction, so each * and + rounds once (R2)."""
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+        subprocess.check_call(["gcc", "-O2", "-std=c99", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
+                               "-o", _SO, _SRC, "-lm"])
+    return _SO
+
+
+class _Desc(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("ncorr", C.c_int32), ("nterms", C.c_int32),
+                ("oversampling", C.c_int32), ("tile", C.c_int32), ("sort_mode", C.c_int32),
+                ("scale_u", C.c_double), ("scale_v", C.c_double), ("n_cf", C.c_int32),
+                ("cf_support", C.c_void_p), ("cf_offset", C.c_void_p), ("cf_data", C.c_void_p)]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+    return _lib
+
+
+def _p(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def max_threads() -> int:
+    return int(lib().lra_ref_max_threads())
+
+
+class RefPlan:
+    """Holds the descriptor (grid dims, CF table, oversampling) the oracle calls share."""
+
+    def __init__(self, nx, ny, ncorr, nterms, oversampling, scale_u, scale_v, cf_support, cf_offset, cf_data,
+                 tile=32, sort_mode=SORT_TILE):
+        self.cf_support = np.ascontiguousarray(cf_support, dtype=np.int32)
+        self.cf_offset = np.ascontiguousarray(cf_offset, dtype=np.int64)
+        self.cf_data = np.ascontiguousarray(cf_data, dtype=np.complex64)
+        self.nx, self.ny, self.ncorr, self.nterms, self.os, self.tile = nx, ny, ncorr, nterms, oversampling, tile
+        self.d = _Desc(nx, ny, ncorr, nterms, oversampling, tile, sort_mode, float(scale_u), float(scale_v),
+                       len(self.cf_support), _p(self.cf_support), _p(self.cf_offset), _p(self.cf_data))
+
+    @property
+    def ntiles(self):
+        T = self.tile
+        return ((self.nx + T - 1) // T) * ((self.ny + T - 1) // T)
+
+    def _geom(self, uvw, freq, cf_index):
+        uvw = np.ascontiguousarray(uvw, dtype=np.float64)
+        freq = np.ascontiguousarray(freq, dtype=np.float64)
+        if cf_index is not None:
+            cf_index = np.ascontiguousarray(cf_index, dtype=np.int32)
+        return uvw, freq, cf_index, uvw.shape[0], freq.shape[0]
+
+    def bin(self, uvw, freq, cf_index=None):
+        uvw, freq, cf_index, nrow, nchan = self._geom(uvw, freq, cf_index)
+        n = nrow * nchan
+        out = dict(ix=np.empty(n, np.int32), iy=np.empty(n, np.int32), fx=np.empty(n, np.int8),
+                   fy=np.empty(n, np.int8), key=np.empty(n, np.uint64), perm=np.empty(n, np.uint32),
+                   tile_start=np.empty(self.ntiles + 1, np.uint32))
+        nv = C.c_int64(0)
+        rc = lib().lra_ref_bin(C.byref(self.d), C.c_int64(nrow), C.c_int32(nchan), _p(uvw), _p(freq), _p(cf_index),
+                               _p(out["ix"]), _p(out["iy"]), _p(out["fx"]), _p(out["fy"]), _p(out["key"]),
+                               _p(out["perm"]), _p(out["tile_start"]), C.byref(nv))
+        assert rc == 0
+        out["n_valid"] = int(nv.value)
+        out["perm"] = out["perm"][: out["n_valid"]]
+        return out
+
+    def grid(self, uvw, freq, cf_index, vis, wt, tau=None, grid=None, sumwt=None, nthreads=0):
+        uvw, freq, cf_index, nrow, nchan = self._geom(uvw, freq, cf_index)
+        vis = np.ascontiguousarray(vis, dtype=np.complex64)
+        wt = np.ascontiguousarray(wt, dtype=np.float32)
+        tau = None if tau is None else np.ascontiguousarray(tau, dtype=np.float32)
+        if grid is None:
+            grid = np.zeros((self.nterms, self.ncorr, self.ny, self.nx), dtype=np.complex128)
+        if sumwt is None:
+            sumwt = np.zeros((self.nterms, self.ncorr), dtype=np.float64)
+        rc = lib().lra_ref_grid(C.byref(self.d), C.c_int64(nrow), C.c_int32(nchan), _p(uvw), _p(freq), _p(cf_index),
+                                _p(vis), _p(wt), _p(tau), _p(grid), _p(sumwt), C.c_int32(nthreads or max_threads()))
+        assert rc == 0
+        return grid, sumwt
+
+    def degrid(self, uvw, freq, cf_index, grid, tau=None, vis_in=None, nthreads=0):
+        uvw, freq, cf_index, nrow, nchan = self._geom(uvw, freq, cf_index)
+        grid = np.ascontiguousarray(grid, dtype=np.complex128)
+        tau = None if tau is None else np.ascontiguousarray(tau, dtype=np.float32)
+        vis_in = None if vis_in is None else np.ascontiguousarray(vis_in, dtype=np.complex64)
+        out = np.empty((nrow, nchan, self.ncorr), dtype=np.complex128)
+        rc = lib().lra_ref_degrid(C.byref(self.d), C.c_int64(nrow), C.c_int32(nchan), _p(uvw), _p(freq), _p(cf_index),
+                                  _p(grid), _p(tau), _p(vis_in), _p(out), C.c_int32(nthreads or max_threads()))
+        assert rc == 0
+        return out
+
+    def grid_pixels(self, uvw, freq, cf_index, vis, wt, tau, pix, nthreads=0):
+        uvw, freq, cf_index, nrow, nchan = self._geom(uvw, freq, cf_index)
+        vis = np.ascontiguousarray(vis, dtype=np.complex64)
+        wt = np.ascontiguousarray(wt, dtype=np.float32)
+        tau = None if tau is None else np.ascontiguousarray(tau, dtype=np.float32)
+        pix = np.ascontiguousarray(pix, dtype=np.int32).reshape(-1, 4)
+        out = np.empty(len(pix), dtype=np.complex128)
+        rc = lib().lra_ref_grid_pixels(C.byref(self.d), C.c_int64(nrow), C.c_int32(nchan), _p(uvw), _p(freq),
+                                       _p(cf_index), _p(vis), _p(wt), _p(tau), C.c_int32(len(pix)), _p(pix), _p(out),
+                                       C.c_int32(nthreads or max_threads()))
+        assert rc == 0
+        return out
+
+    def degrid_points(self, uvw, freq, cf_index, grid_c64, tau, vis_in, sel):
+        uvw, freq, cf_index, nrow, nchan = self._geom(uvw, freq, cf_index)
+        grid_c64 = np.ascontiguousarray(grid_c64, dtype=np.complex64)
+        tau = None if tau is None else np.ascontiguousarray(tau, dtype=np.float32)
+        vis_in = None if vis_in is None else np.ascontiguousarray(vis_in, dtype=np.complex64)
+        sel = np.ascontiguousarray(sel, dtype=np.int64)
+        out = np.empty((len(sel), self.ncorr), dtype=np.complex128)
+        rc = lib().lra_ref_degrid_points(C.byref(self.d), C.c_int64(nrow), C.c_int32(nchan), _p(uvw), _p(freq),
+                                         _p(cf_index), _p(grid_c64), _p(tau), _p(vis_in), C.c_int32(len(sel)),
+                                         _p(sel), _p(out))
+        assert rc == 0
+        return out
+
+
+def plan_for(wl, nterms=None, sort_mode=SORT_TILE, tile=None) -> RefPlan:
+    """RefPlan for a ``workloads.Workload`` (argument marshalling only)."""
+    c = wl.cfg
+    return RefPlan(c.nx, c.ny, c.ncorr, c.nterms if nterms is None else nterms, c.oversampling, wl.scale_u,
+                   wl.scale_v, wl.cf.support, wl.cf.offset, wl.cf.data, tile=tile or c.tile, sort_mode=sort_mode)
