@@ -433,8 +433,8 @@ def test_prolate_is_the_dominant_band_limited_eigenfunction():
         assert 1.0 - 1e-6 < lam < 1.0 + 1e-12 and resid < 1e-10
         x = np.linspace(-1, 1, 201)
         v = psi(x)
-        assert (v > 0).all() and np.abs(v - v[::-1]).max() < 1e-12 and v.argmax() == 100
-        assert (np.diff(v[100:]) < 0).all()
+        assert (v > -1e-12).all() and np.abs(v - v[::-1]).max() < 1e-12 and v.argmax() == 100
+        assert (np.diff(v[100:]) < 1e-12).all()
         assert v[0] / v[100] < 1e-3
 
 
