@@ -1,0 +1,133 @@
+/* lra.h -- C ABI of liblra: gridding (G) and degridding (D) of radio-interferometric visibilities on
+ * one NVIDIA B200 (sm_100a).
+ *
+ * Operations (arxiv 2508.17187; line numbers are /root/reference/PAPER.md):
+ *   G(c_ij): resample irregularly sampled weighted visibilities onto the regular uv grid, "accumulation
+ *            on a grid at the pixel corresponding to u_ij"            -- Eq. 7
+ *   D(c_ij): the reverse operator, resampling the gridded model at the visibility coordinates
+ *            (model prediction V^Mod)                                 -- Eq. 6
+ *   W_ij [V - V^Mod]: weights outside G, residual between D and G     -- Eq. 23 / 26
+ *   c_ij = CF_ij(nu, w, t): "in practice a kernel applies to a set of data points"; the caller picks the
+ *            kernel of every visibility point through cf_index        -- Eq. 27
+ *   re-ordering of the data for runtime performance (PreSolvePrep / InLoopPrep)  -- PAPER.md:345, 429
+ *   one-time caching of the kernels (PreCompute)                      -- PAPER.md:207, 335-343, 380
+ * The resampling arithmetic the paper leaves open is fixed by readings R1..R15 in DESIGN.md.
+ *
+ * Call chain:  lra_plan_create -> lra_bin -> lra_grid / lra_degrid (any number, any order) -> lra_plan_destroy
+ *
+ * Conventions
+ *   - "device" pointers are CUDA device memory on the plan's device, owned by the caller (e.g. allocated by
+ *     PyTorch); the library never frees them and does not keep them past the stream work of the call that
+ *     received them -- EXCEPT the geometry arrays given to lra_bin (uvw_m is not kept; see lra_bin).
+ *   - "host" pointers are ordinary host memory, read during the call only.
+ *   - Every call returns an lra_status.  No exceptions cross the ABI.  Calls enqueue work on the plan's
+ *     stream and return without synchronising unless stated otherwise.
+ *   - A visibility point k = r*nchan + c is one (row, channel); its ncorr samples share position and kernel.
+ *   - complex64 = two consecutive floats (re, im).
+ */
+#ifndef LRA_H_
+#define LRA_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  LRA_OK = 0,
+  LRA_EINVAL = 1, /* bad argument (null pointer, size out of range, even support, ...) */
+  LRA_ENOMEM = 2, /* host or device allocation failed                                   */
+  LRA_ECUDA = 3,  /* a CUDA runtime call failed; see lra_last_cuda_error                */
+  LRA_ESTATE = 4  /* call out of order (lra_grid before lra_bin, ...)                   */
+} lra_status;
+
+enum { LRA_SORT_TILE = 0, LRA_SORT_TILE_CF = 1 };
+
+typedef struct lra_plan lra_plan; /* opaque */
+
+typedef struct {
+  int32_t nx, ny;         /* grid size in pixels; u along x (fastest), v along y; origin pixel (nx/2, ny/2) [R1] */
+  int32_t ncorr, nterms;  /* grids per call = nterms*ncorr; 1 <= ncorr <= 4, 1 <= nterms <= 4                  */
+  int32_t oversampling;   /* os >= 1: sub-pixel phases per pixel of the CF table [R3]                        */
+  int32_t tile;           /* T: uv-tile edge in pixels used by the bucket sort, power of two >= 8 (default 32)   */
+  int32_t sort_mode;      /* LRA_SORT_TILE | LRA_SORT_TILE_CF [R5]                                             */
+  double scale_u, scale_v; /* pixels per wavelength along u and v; sign allowed [R1]                            */
+  int32_t n_cf;           /* number of kernels in the CF table                                                 */
+  const int32_t* cf_support; /* host [n_cf]: support S_c in pixels, odd, 1 <= S_c <= 129                        */
+  const int64_t* cf_offset;  /* host [n_cf]: element (complex64) offset of kernel c inside cf_data              */
+  const void* cf_data;    /* host, complex64: kernel c is (S_c*os)^2 samples, row-major, v slow; sample m of a
+                             row sits (m - c0)/os pixels from the kernel centre, c0 = h*os + (os-1-os/2) [R3]   */
+  int32_t device;         /* CUDA device ordinal                                                               */
+  void* stream;           /* cudaStream_t all work of this plan is enqueued on (NULL = legacy default stream)  */
+} lra_plan_desc;
+
+/* PreCompute: validates the descriptor, copies the CF table to the device and re-lays
+ * every oversampled kernel into phase-major slabs [cf][fy][fx][S][S] so that the S*S taps one visibility
+ * point needs are contiguous.  Synchronises the plan's stream before returning (the host table may be freed).
+ * Errors: LRA_EINVAL, LRA_ENOMEM, LRA_ECUDA.  *out is NULL on failure. */
+int lra_plan_create(lra_plan** out, const lra_plan_desc* desc);
+
+/* Frees everything the plan owns (CF slabs, bin arrays, scratch).  Synchronises the plan's stream. */
+int lra_plan_destroy(lra_plan* p);
+
+/* Re-ordering: for every visibility point computes grid pixel (ix, iy), sub-pixel phase
+ * (fx, fy), validity [R2, R4] and the sort key [R5], then stable-sorts the valid point indices by key and
+ * records per-tile start offsets.  The result stays in the plan and is consumed by lra_grid / lra_degrid.
+ *   nrow, nchan : npoints = nrow*nchan must be < 2^31
+ *   uvw_m       : device double [nrow][3], baseline coordinates in metres
+ *   freq_hz     : HOST double [nchan]  (small; the per-channel scale (freq/c)*scale is formed on the host)
+ *   cf_index    : device int32 [nrow][nchan] kernel of every point, or NULL (=> kernel 0)
+ * The input arrays are not referenced after the call's stream work completes.
+ * Errors: LRA_EINVAL, LRA_ENOMEM (growing the plan's bin arrays), LRA_ECUDA. */
+int lra_bin(lra_plan* p, int64_t nrow, int32_t nchan, const double* uvw_m, const double* freq_hz,
+            const int32_t* cf_index);
+
+/* Copies the bin result out for checking (all device pointers, each may be NULL to skip it):
+ *   ix, iy int32 [npoints], fx, fy int8 [npoints], key uint64 [npoints]  (invalid point: ix = iy = -1,
+ *   fx = fy = 0, key = 2^64-1); perm uint32 [npoints] (first n_valid entries meaningful);
+ *   tile_start uint32 [ntiles+1], ntiles = ceil(nx/T)*ceil(ny/T); n_valid: HOST int64.
+ * Synchronises the plan's stream.  Errors: LRA_ESTATE before lra_bin. */
+int lra_bin_export(lra_plan* p, int32_t* ix, int32_t* iy, int8_t* fx, int8_t* fy, uint64_t* key, uint32_t* perm,
+                   uint32_t* tile_start, int64_t* n_valid);
+
+/* Gridding (Eq. 7 with the weights of Eq. 23):
+ *   grid[t][p][iy+j][ix+i] += CF[cf][fy][fx][j][i] * (wt[k][p] * tau[c][t] * vis[k][p])   for all taps (j, i)
+ *   sumwt[t][p]            += wt[k][p] * tau[c][t]                                         [R6]
+ * over the valid points of the last lra_bin.  fp32 multiply-add, fp32 accumulation.
+ *   vis_c64  : device complex64 [nrow][nchan][ncorr]
+ *   wt       : device float [nrow][nchan][ncorr]   (flags are expressed as weight 0 [R4])
+ *   tau      : device float [nchan][nterms] Taylor weights, or NULL (=> 1) [R11]
+ *   grid_c64 : device complex64 [nterms][ncorr][ny][nx], ACCUMULATED INTO (caller zeroes it)
+ *   sumwt    : device double [nterms][ncorr], accumulated into; may be NULL
+ * Errors: LRA_ESTATE before lra_bin, LRA_EINVAL, LRA_ECUDA. */
+int lra_grid(lra_plan* p, const void* vis_c64, const float* wt, const float* tau, void* grid_c64, double* sumwt);
+
+/* Degridding (Eq. 6; exact adjoint of lra_grid with unit weights [R7]):
+ *   V[k][p] = sum_t tau[c][t] * sum_{j,i} conj(CF[cf][fy][fx][j][i]) * grid[t][p][iy+j][ix+i]
+ *   vis_out[k][p] = vis_in ? vis_in[k][p] - V[k][p] : V[k][p]        (fused residual of Eq. 23)
+ * Invalid points get V = 0.  vis_out is overwritten for ALL nrow*nchan*ncorr samples.
+ *   grid_c64   : device complex64 [nterms][ncorr][ny][nx], read only
+ *   vis_in_c64 : device complex64 [nrow][nchan][ncorr] or NULL;  vis_out_c64: device, same shape
+ *                (vis_out may alias vis_in)
+ * Errors: LRA_ESTATE before lra_bin, LRA_EINVAL, LRA_ECUDA. */
+int lra_degrid(lra_plan* p, const void* grid_c64, const float* tau, const void* vis_in_c64, void* vis_out_c64);
+
+/* Number of kernel launches the plan has enqueued since creation (for bench.py's gpu_launches). */
+int64_t lra_launch_count(const lra_plan* p);
+
+/* Sum over the valid points of the last lra_bin of S^2 (taps per correlation and term); synchronises. */
+int lra_tap_count(lra_plan* p, int64_t* n_valid, int64_t* sum_s2);
+
+/* Selects the gridding / degridding kernel variant: 0 = default (fastest verified), other values are
+ * listed in DESIGN.md (1 = plain global-atomic gridder kept as the "before" profile). */
+int lra_set_variant(lra_plan* p, int32_t grid_variant, int32_t degrid_variant);
+
+const char* lra_strerror(int code);
+/* cudaGetErrorString of the last failing CUDA call of this plan ("" if none). */
+const char* lra_last_cuda_error(const lra_plan* p);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LRA_H_ */

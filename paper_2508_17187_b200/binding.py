@@ -1,0 +1,156 @@
+"""Thin Python binding of liblra.so (include/lra.h).  Argument marshalling only: every step of the path
+runs in the CUDA kernels behind the C ABI.  PyTorch supplies device memory and streams, nothing else.
+
+The functions carry the names of the C entry points and take torch CUDA tensors (device pointers) or
+numpy arrays (host pointers) exactly where lra.h says "device" or "host".  There is no CPU fallback: if the
+shared library cannot be loaded, importing this module's `lib()` raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+
+from . import _build
+
+LRA_OK, LRA_EINVAL, LRA_ENOMEM, LRA_ECUDA, LRA_ESTATE = 0, 1, 2, 3, 4
+LRA_SORT_TILE, LRA_SORT_TILE_CF = 0, 1
+
+
+class LraError(RuntimeError):
+    pass
+
+
+class lra_plan_desc(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("ncorr", C.c_int32), ("nterms", C.c_int32),
+                ("oversampling", C.c_int32), ("tile", C.c_int32), ("sort_mode", C.c_int32),
+                ("scale_u", C.c_double), ("scale_v", C.c_double), ("n_cf", C.c_int32),
+                ("cf_support", C.c_void_p), ("cf_offset", C.c_void_p), ("cf_data", C.c_void_p),
+                ("device", C.c_int32), ("stream", C.c_void_p)]
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Loads liblra.so (building it in-tree with nvcc if sources are newer).  Fails loudly otherwise."""
+    global _lib
+    if _lib is None:
+        path = _build.SO_PATH
+        if _build.needs_build():
+            path = _build.build()
+        if not os.path.exists(path):
+            raise LraError(f"liblra.so not found at {path}; the CUDA extension is required (no CPU fallback)")
+        L = C.CDLL(path)
+        vp, i32, i64 = C.c_void_p, C.c_int32, C.c_int64
+        L.lra_plan_create.argtypes = [C.POINTER(vp), C.POINTER(lra_plan_desc)]
+        L.lra_plan_destroy.argtypes = [vp]
+        L.lra_bin.argtypes = [vp, i64, i32, vp, vp, vp]
+        L.lra_bin_export.argtypes = [vp] * 8 + [C.POINTER(i64)]
+        L.lra_grid.argtypes = [vp] * 6
+        L.lra_degrid.argtypes = [vp] * 5
+        L.lra_launch_count.argtypes = [vp]
+        L.lra_launch_count.restype = i64
+        L.lra_tap_count.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
+        L.lra_set_variant.argtypes = [vp, i32, i32]
+        L.lra_strerror.argtypes = [C.c_int]
+        L.lra_strerror.restype = C.c_char_p
+        L.lra_last_cuda_error.argtypes = [vp]
+        L.lra_last_cuda_error.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+EXPORTED = ["lra_plan_create", "lra_plan_destroy", "lra_bin", "lra_bin_export", "lra_grid", "lra_degrid",
+            "lra_launch_count", "lra_tap_count", "lra_set_variant", "lra_strerror", "lra_last_cuda_error"]
+
+
+def _check(rc: int, plan=None):
+    if rc != LRA_OK:
+        msg = lib().lra_strerror(rc).decode()
+        if plan:
+            detail = lib().lra_last_cuda_error(plan).decode()
+            if detail:
+                msg += f" ({detail})"
+        raise LraError(f"liblra: {msg} [code {rc}]")
+
+
+def _dev(t, dtype=None) -> Optional[int]:
+    """Device pointer of a contiguous CUDA tensor (None passes NULL)."""
+    if t is None:
+        return None
+    if not t.is_cuda or not t.is_contiguous():
+        raise LraError("expected a contiguous CUDA tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise LraError(f"expected dtype {dtype}, got {t.dtype}")
+    return t.data_ptr()
+
+
+def _host(a: np.ndarray, dtype) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=dtype)
+
+
+def lra_plan_create(nx, ny, ncorr, nterms, oversampling, scale_u, scale_v, cf_support, cf_offset, cf_data,
+                    tile=32, sort_mode=LRA_SORT_TILE_CF, device=0, stream=None) -> int:
+    """-> opaque plan handle (int).  cf_* are HOST numpy arrays (lra.h: lra_plan_desc)."""
+    sup = _host(cf_support, np.int32)
+    off = _host(cf_offset, np.int64)
+    dat = _host(cf_data, np.complex64)
+    d = lra_plan_desc(nx, ny, ncorr, nterms, oversampling, tile, sort_mode, float(scale_u), float(scale_v), len(sup),
+                      sup.ctypes.data, off.ctypes.data, dat.ctypes.data, device, stream or 0)
+    h = C.c_void_p()
+    _check(lib().lra_plan_create(C.byref(h), C.byref(d)))
+    return h.value
+
+
+def lra_plan_destroy(plan: int):
+    _check(lib().lra_plan_destroy(plan))
+
+
+def lra_bin(plan: int, uvw_m, freq_hz, cf_index=None):
+    """uvw_m: CUDA float64 [nrow, 3]; freq_hz: HOST float64 [nchan]; cf_index: CUDA int32 [nrow, nchan] or None."""
+    import torch
+    f = _host(freq_hz, np.float64)
+    nrow, nchan = int(uvw_m.shape[0]), len(f)
+    _check(lib().lra_bin(plan, nrow, nchan, _dev(uvw_m, torch.float64), f.ctypes.data, _dev(cf_index, torch.int32)), plan)
+
+
+def lra_bin_export(plan: int, ix=None, iy=None, fx=None, fy=None, key=None, perm=None, tile_start=None) -> int:
+    """Copies the bin arrays into the given CUDA tensors (None skips); returns n_valid."""
+    nv = C.c_int64(0)
+    _check(lib().lra_bin_export(plan, _dev(ix), _dev(iy), _dev(fx), _dev(fy), _dev(key), _dev(perm), _dev(tile_start),
+                                C.byref(nv)), plan)
+    return int(nv.value)
+
+
+def lra_grid(plan: int, vis, wt, tau, grid, sumwt=None):
+    import torch
+    _check(lib().lra_grid(plan, _dev(vis, torch.complex64), _dev(wt, torch.float32), _dev(tau, torch.float32),
+                          _dev(grid, torch.complex64), _dev(sumwt, torch.float64)), plan)
+
+
+def lra_degrid(plan: int, grid, tau, vis_in, vis_out):
+    import torch
+    _check(lib().lra_degrid(plan, _dev(grid, torch.complex64), _dev(tau, torch.float32), _dev(vis_in, torch.complex64),
+                            _dev(vis_out, torch.complex64)), plan)
+
+
+def lra_launch_count(plan: int) -> int:
+    return int(lib().lra_launch_count(plan))
+
+
+def lra_tap_count(plan: int):
+    """-> (n_valid, sum over valid points of S^2)."""
+    a, b = C.c_int64(0), C.c_int64(0)
+    _check(lib().lra_tap_count(plan, C.byref(a), C.byref(b)), plan)
+    return int(a.value), int(b.value)
+
+
+def lra_set_variant(plan: int, grid_variant: int = 0, degrid_variant: int = 0):
+    _check(lib().lra_set_variant(plan, grid_variant, degrid_variant), plan)
+
+
+def lra_strerror(code: int) -> str:
+    return lib().lra_strerror(code).decode()

@@ -1,0 +1,178 @@
+// lra_plan.cu -- plan life cycle, CF ingest (PreCompute) and the thin C-ABI entry
+// points that validate arguments and forward to the kernels' host drivers.
+#include <new>
+#include <string.h>
+
+#include "lra_internal.cuh"
+
+// Re-lay one oversampled kernel into phase-major slabs (reading R3):
+//   slab(fyi, fxi)[j + h][i + h] = K[(j*os - fy) + c0][(i*os - fx) + c0],  fy = fyi - os/2, c0 = h*os + (os-1-os/2)
+// One thread per slab element; padding elements (slab_stride > S*S) are zero-filled.
+__global__ void lra_relayout_kernel(const float2* __restrict__ K, float2* __restrict__ slab, int S, int os,
+                                    int slab_stride) {
+  const int h = (S - 1) / 2;
+  const int c0 = h * os + (os - 1 - os / 2);
+  const int64_t n = (int64_t)os * os * slab_stride;
+  const int64_t ld = (int64_t)S * os;
+  for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
+    int phase = (int)(e / slab_stride), t = (int)(e % slab_stride);
+    float2 v = make_float2(0.f, 0.f);
+    if (t < S * S) {
+      int fyi = phase / os, fxi = phase % os;
+      int j = t / S - h, i = t % S - h;
+      int row = j * os - (fyi - os / 2) + c0, col = i * os - (fxi - os / 2) + c0;
+      v = K[row * ld + col];
+    }
+    slab[e] = v;
+  }
+}
+
+static int is_pow2(int x) { return x > 0 && (x & (x - 1)) == 0; }
+
+extern "C" int lra_plan_create(lra_plan** out, const lra_plan_desc* d) {
+  if (!out) return LRA_EINVAL;
+  *out = nullptr;
+  if (!d || d->nx < 1 || d->ny < 1 || d->nx > 32768 || d->ny > 32768) return LRA_EINVAL;
+  if (d->ncorr < 1 || d->ncorr > 4 || d->nterms < 1 || d->nterms > 4) return LRA_EINVAL;
+  if (d->oversampling < 1 || d->oversampling > 64) return LRA_EINVAL;
+  int tile = d->tile == 0 ? 32 : d->tile;
+  if (!is_pow2(tile) || tile < 8 || tile > 1024) return LRA_EINVAL;
+  if (d->sort_mode != LRA_SORT_TILE && d->sort_mode != LRA_SORT_TILE_CF) return LRA_EINVAL;
+  if (d->n_cf < 1 || d->n_cf > (1 << 24) || !d->cf_support || !d->cf_offset || !d->cf_data) return LRA_EINVAL;
+  if (!(d->scale_u == d->scale_u) || !(d->scale_v == d->scale_v)) return LRA_EINVAL;
+  for (int c = 0; c < d->n_cf; ++c) {
+    int S = d->cf_support[c];
+    if (S < 1 || S > 129 || (S & 1) == 0 || d->cf_offset[c] < 0) return LRA_EINVAL;
+  }
+  lra_plan* p = new (std::nothrow) lra_plan();
+  if (!p) return LRA_ENOMEM;
+  p->nx = d->nx; p->ny = d->ny; p->ncorr = d->ncorr; p->nterms = d->nterms; p->os = d->oversampling;
+  p->tile = tile; p->sort_mode = d->sort_mode; p->n_cf = d->n_cf;
+  p->scale_u = d->scale_u; p->scale_v = d->scale_v;
+  p->device = d->device; p->stream = (cudaStream_t)d->stream;
+  p->ntx = (p->nx + tile - 1) / tile; p->nty = (p->ny + tile - 1) / tile; p->ntiles = p->ntx * p->nty;
+  p->last_err = cudaSuccess;
+  p->cf_support.assign(d->cf_support, d->cf_support + d->n_cf);
+  p->slab_off.resize(d->n_cf);
+  p->slab_stride.resize(d->n_cf);
+  int64_t total = 0, max_in = 0;
+  p->max_support = 1;
+  for (int c = 0; c < d->n_cf; ++c) {
+    int S = p->cf_support[c];
+    p->slab_stride[c] = (S * S + 1) & ~1;
+    p->slab_off[c] = total;
+    total += (int64_t)p->os * p->os * p->slab_stride[c];
+    int64_t n_in = (int64_t)S * p->os * S * p->os;
+    if (n_in > max_in) max_in = n_in;
+    if (S > p->max_support) p->max_support = S;
+  }
+  if ((total >> 1) >= (int64_t)1 << 32) { delete p; return LRA_EINVAL; }
+  p->slab_elems = total;
+
+  float2* staging = nullptr;
+  auto fail = [&](int code) { if (staging) cudaFree(staging); lra_plan_destroy(p); return code; };
+#define CK(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { p->last_err = e__; \
+    return fail(e__ == cudaErrorMemoryAllocation ? LRA_ENOMEM : LRA_ECUDA); } } while (0)
+  CK(cudaSetDevice(p->device));
+  CK(cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, p->device));
+  CK(cudaMalloc(&p->slabs, (size_t)total * sizeof(float2)));
+  CK(cudaMalloc(&p->d_cf_support, (size_t)d->n_cf * sizeof(int32_t)));
+  CK(cudaMalloc(&p->d_slab_off, (size_t)d->n_cf * sizeof(int64_t)));
+  CK(cudaMalloc(&p->counters, 64 * sizeof(unsigned long long)));
+  CK(cudaMalloc(&p->tile_start, (size_t)(p->ntiles + 1) * sizeof(uint32_t)));
+  CK(cudaMemcpyAsync(p->d_cf_support, p->cf_support.data(), (size_t)d->n_cf * sizeof(int32_t), cudaMemcpyHostToDevice, p->stream));
+  CK(cudaMemcpyAsync(p->d_slab_off, p->slab_off.data(), (size_t)d->n_cf * sizeof(int64_t), cudaMemcpyHostToDevice, p->stream));
+  // Kernels are staged one at a time through a buffer sized for the largest, so the device never holds two
+  // copies of a large table (cfg4: 616 MB).
+  CK(cudaMalloc(&staging, (size_t)max_in * sizeof(float2)));
+  for (int c = 0; c < d->n_cf; ++c) {
+    int S = p->cf_support[c];
+    int64_t n_in = (int64_t)S * p->os * S * p->os;
+    const float2* src = (const float2*)d->cf_data + d->cf_offset[c];
+    CK(cudaMemcpyAsync(staging, src, (size_t)n_in * sizeof(float2), cudaMemcpyHostToDevice, p->stream));
+    int64_t n_out = (int64_t)p->os * p->os * p->slab_stride[c];
+    int blocks = (int)((n_out + 255) / 256);
+    if (blocks > 4096) blocks = 4096;
+    lra_relayout_kernel<<<blocks, 256, 0, p->stream>>>(staging, p->slabs + p->slab_off[c], S, p->os, p->slab_stride[c]);
+    p->launches++;
+    CK(cudaGetLastError());
+  }
+  CK(cudaStreamSynchronize(p->stream));
+  cudaFree(staging);
+  staging = nullptr;
+#undef CK
+  *out = p;
+  return LRA_OK;
+}
+
+extern "C" int lra_plan_destroy(lra_plan* p) {
+  if (!p) return LRA_EINVAL;
+  cudaSetDevice(p->device);
+  cudaStreamSynchronize(p->stream);
+  void* ptrs[] = {p->slabs, p->d_cf_support, p->d_slab_off, p->ix, p->iy, p->fx, p->fy, p->key, p->skey[0], p->skey[1],
+                  p->sval[0], p->sval[1], p->hist, p->tile_start, p->rec, p->counters, p->d_su, p->d_sv, p->work, p->item_off};
+  for (void* q : ptrs)
+    if (q) cudaFree(q);
+  delete p;
+  return LRA_OK;
+}
+
+extern "C" int lra_bin(lra_plan* p, int64_t nrow, int32_t nchan, const double* uvw_m, const double* freq_hz,
+                       const int32_t* cf_index) {
+  if (!p || nrow < 0 || nchan < 1 || (nrow > 0 && !uvw_m) || !freq_hz) return LRA_EINVAL;
+  if (nrow * (int64_t)nchan >= ((int64_t)1 << 31)) return LRA_EINVAL;
+  LRA_CUDA(p, cudaSetDevice(p->device));
+  return lra_bin_impl(p, nrow, nchan, uvw_m, freq_hz, cf_index);
+}
+
+extern "C" int lra_grid(lra_plan* p, const void* vis, const float* wt, const float* tau, void* grid, double* sumwt) {
+  if (!p) return LRA_EINVAL;
+  if (!p->binned) return LRA_ESTATE;
+  if (!grid || (p->npoints > 0 && (!vis || !wt))) return LRA_EINVAL;
+  LRA_CUDA(p, cudaSetDevice(p->device));
+  return lra_grid_impl(p, (const float2*)vis, wt, tau, (float2*)grid, sumwt);
+}
+
+extern "C" int lra_degrid(lra_plan* p, const void* grid, const float* tau, const void* vis_in, void* vis_out) {
+  if (!p) return LRA_EINVAL;
+  if (!p->binned) return LRA_ESTATE;
+  if (!grid || (p->npoints > 0 && !vis_out)) return LRA_EINVAL;
+  LRA_CUDA(p, cudaSetDevice(p->device));
+  return lra_degrid_impl(p, (const float2*)grid, tau, (const float2*)vis_in, (float2*)vis_out);
+}
+
+extern "C" int64_t lra_launch_count(const lra_plan* p) { return p ? p->launches : 0; }
+
+extern "C" int lra_tap_count(lra_plan* p, int64_t* n_valid, int64_t* sum_s2) {
+  if (!p) return LRA_EINVAL;
+  if (!p->binned) return LRA_ESTATE;
+  unsigned long long h[2];
+  LRA_CUDA(p, cudaMemcpyAsync(h, p->counters, sizeof h, cudaMemcpyDeviceToHost, p->stream));
+  LRA_CUDA(p, cudaStreamSynchronize(p->stream));
+  if (n_valid) *n_valid = (int64_t)h[0];
+  if (sum_s2) *sum_s2 = (int64_t)h[1];
+  return LRA_OK;
+}
+
+extern "C" int lra_set_variant(lra_plan* p, int32_t grid_variant, int32_t degrid_variant) {
+  if (!p || grid_variant < 0 || grid_variant > 3 || degrid_variant < 0 || degrid_variant > 3) return LRA_EINVAL;
+  p->grid_variant = grid_variant;
+  p->degrid_variant = degrid_variant;
+  return LRA_OK;
+}
+
+extern "C" const char* lra_strerror(int code) {
+  switch (code) {
+    case LRA_OK: return "ok";
+    case LRA_EINVAL: return "invalid argument";
+    case LRA_ENOMEM: return "out of memory";
+    case LRA_ECUDA: return "CUDA error";
+    case LRA_ESTATE: return "call out of order (lra_bin first)";
+    default: return "unknown error";
+  }
+}
+
+extern "C" const char* lra_last_cuda_error(const lra_plan* p) {
+  if (!p || p->last_err == cudaSuccess) return "";
+  return cudaGetErrorString(p->last_err);
+}

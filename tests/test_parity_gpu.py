@@ -1,0 +1,256 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same seeded
+inputs.  Tolerances are north_star's: bin outputs bit-exact; grid / degridded visibilities relative L2 <= 1e-5 and
+max abs <= 1e-4 * max|.|; sumwt relative <= 1e-6."""
+import numpy as np
+import pytest
+
+from paper_2508_17187_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+C_LIGHT = 299792458.0
+
+
+@pytest.fixture(scope="module")
+def B():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2508_17187_b200 import binding
+    binding.lib()
+    return binding
+
+
+def dev(a):
+    return None if a is None else torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+class GpuRun:
+    """One plan + bin on the GPU for a Workload-like bundle of numpy inputs."""
+
+    def __init__(self, B, nx, ny, ncorr, nterms, os_, su, sv, sup, off, data, uvw, freq, cf_index, tile=32, sort_mode=1):
+        self.B = B
+        self.shape = (nterms, ncorr, ny, nx)
+        self.plan = B.lra_plan_create(nx, ny, ncorr, nterms, os_, su, sv, sup, off, data, tile=tile, sort_mode=sort_mode)
+        self.nrow, self.nchan, self.ncorr = len(uvw), len(freq), ncorr
+        self.ntiles = ((nx + tile - 1) // tile) * ((ny + tile - 1) // tile)
+        self.uvw, self.cfi = dev(uvw), dev(cf_index)
+        B.lra_bin(self.plan, self.uvw, freq, self.cfi)
+
+    def export(self):
+        n = self.nrow * self.nchan
+        o = dict(ix=torch.empty(n, dtype=torch.int32, device="cuda"), iy=torch.empty(n, dtype=torch.int32, device="cuda"),
+                 fx=torch.empty(n, dtype=torch.int8, device="cuda"), fy=torch.empty(n, dtype=torch.int8, device="cuda"),
+                 key=torch.empty(n, dtype=torch.int64, device="cuda"), perm=torch.empty(n, dtype=torch.int32, device="cuda"),
+                 tile_start=torch.empty(self.ntiles + 1, dtype=torch.int32, device="cuda"))
+        nv = self.B.lra_bin_export(self.plan, **o)
+        out = {k: v.cpu().numpy() for k, v in o.items()}
+        out["key"] = out["key"].view(np.uint64)
+        out["perm"] = out["perm"].view(np.uint32)[:nv]
+        out["tile_start"] = out["tile_start"].view(np.uint32)
+        out["n_valid"] = nv
+        return out
+
+    def grid(self, vis, wt, tau=None, variant=0, grid0=None):
+        self.B.lra_set_variant(self.plan, variant, 0)
+        g = torch.zeros(self.shape, dtype=torch.complex64, device="cuda") if grid0 is None else dev(grid0)
+        sw = torch.zeros(self.shape[:2], dtype=torch.float64, device="cuda")
+        self.B.lra_grid(self.plan, dev(vis), dev(wt), dev(tau), g, sw)
+        torch.cuda.synchronize()
+        return g.cpu().numpy(), sw.cpu().numpy()
+
+    def degrid(self, grid, tau=None, vis_in=None):
+        out = torch.full((self.nrow, self.nchan, self.ncorr), 7.0 + 7.0j, dtype=torch.complex64, device="cuda")
+        self.B.lra_degrid(self.plan, dev(grid.astype(np.complex64)), dev(tau), dev(vis_in), out)
+        torch.cuda.synchronize()
+        return out.cpu().numpy()
+
+    def close(self):
+        self.B.lra_plan_destroy(self.plan)
+
+
+def run_for(B, wl, nterms=None, sort_mode=1, tile=32):
+    c = wl.cfg
+    return GpuRun(B, c.nx, c.ny, c.ncorr, c.nterms if nterms is None else nterms, c.oversampling, wl.scale_u, wl.scale_v,
+                  wl.cf.support, wl.cf.offset, wl.cf.data, wl.uvw, wl.freq, wl.cf_index, tile=tile, sort_mode=sort_mode)
+
+
+def assert_close(got, want, what):
+    want = np.asarray(want, dtype=np.complex128)
+    got = np.asarray(got, dtype=np.complex128)
+    scale = np.abs(want).max()
+    assert scale > 0, what
+    l2 = np.linalg.norm((got - want).ravel()) / np.linalg.norm(want.ravel())
+    mx = np.abs(got - want).max()
+    assert l2 <= 1e-5, f"{what}: relative L2 {l2:.3e}"
+    assert mx <= 1e-4 * scale, f"{what}: max abs {mx:.3e} vs scale {scale:.3e}"
+
+
+def assert_bin_equal(g, r):
+    assert g["n_valid"] == r["n_valid"]
+    for k in ("ix", "iy", "fx", "fy", "key", "perm", "tile_start"):
+        assert np.array_equal(g[k], r[k]), k
+
+
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n", [1, 2, 3, 4, 5])
+@pytest.mark.parametrize("mode", [0, 1])
+def test_bin_bit_exact(B, ref, n, mode):
+    wl = W.make_workload(W.small_config(n))
+    run = run_for(B, wl, sort_mode=mode)
+    try:
+        assert_bin_equal(run.export(), ref.plan_for(wl, sort_mode=mode).bin(wl.uvw, wl.freq, wl.cf_index))
+    finally:
+        run.close()
+
+
+def test_bin_invalid_points_and_small_tile(B, ref):
+    wl = W.make_workload(W.small_config(3))
+    uvw, cfi = wl.uvw.copy(), wl.cf_index.copy()
+    uvw[5] = [3.0e5, -2.0e5, 10.0]
+    uvw[17, 0] = np.nan
+    uvw[23, 1] = np.inf
+    uvw[29, 0] = 1e300
+    cfi[40, 1] = -1
+    cfi[41, 2] = wl.cfg.n_cf
+    for tile, mode in ((8, 1), (16, 0), (64, 1)):
+        c = wl.cfg
+        run = GpuRun(B, c.nx, c.ny, c.ncorr, 1, c.oversampling, wl.scale_u, -wl.scale_v, wl.cf.support, wl.cf.offset,
+                     wl.cf.data, uvw, wl.freq, cfi, tile=tile, sort_mode=mode)
+        try:
+            r = ref.RefPlan(c.nx, c.ny, c.ncorr, 1, c.oversampling, wl.scale_u, -wl.scale_v, wl.cf.support, wl.cf.offset,
+                            wl.cf.data, tile=tile, sort_mode=mode)
+            want = r.bin(uvw, wl.freq, cfi)
+            assert want["n_valid"] < c.npoints
+            assert_bin_equal(run.export(), want)
+        finally:
+            run.close()
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 4, 5])
+def test_grid_parity_small_configs(B, ref, n):
+    wl = W.make_workload(W.small_config(n))
+    rp = ref.plan_for(wl)
+    want, want_sw = rp.grid(wl.uvw, wl.freq, wl.cf_index, wl.vis, wl.wt, wl.tau)
+    run = run_for(B, wl)
+    try:
+        for variant in (0, 1):
+            got, sw = run.grid(wl.vis, wl.wt, wl.tau, variant=variant)
+            assert_close(got, want, f"cfg{n} grid variant {variant}")
+            assert np.abs(sw - want_sw).max() <= 1e-6 * np.abs(want_sw).max()
+        nv, s2 = B.lra_tap_count(run.plan)
+        assert nv == rp.bin(wl.uvw, wl.freq, wl.cf_index)["n_valid"] and s2 > 0
+    finally:
+        run.close()
+
+
+@pytest.mark.parametrize("n", [1, 3, 4, 5])
+def test_degrid_parity_small_configs(B, ref, n):
+    wl = W.make_workload(W.small_config(n))
+    rng = np.random.default_rng(40 + n)
+    c = wl.cfg
+    if wl.model_grid is not None and c.nterms == 1:
+        g = wl.model_grid
+    else:
+        g = (rng.standard_normal((c.nterms, c.ncorr, c.ny, c.nx)) + 1j * rng.standard_normal((c.nterms, c.ncorr, c.ny, c.nx))).astype(np.complex64)
+    rp = ref.plan_for(wl)
+    run = run_for(B, wl)
+    try:
+        want = rp.degrid(wl.uvw, wl.freq, wl.cf_index, g.astype(np.complex128), wl.tau)
+        assert_close(run.degrid(g, wl.tau), want, f"cfg{n} degrid")
+        want_res = rp.degrid(wl.uvw, wl.freq, wl.cf_index, g.astype(np.complex128), wl.tau, vis_in=wl.vis)
+        assert_close(run.degrid(g, wl.tau, vis_in=wl.vis), want_res, f"cfg{n} degrid residual")
+    finally:
+        run.close()
+
+
+def test_cfg5_pipeline_degrid_then_multiterm_grid(B, ref):
+    """Config 5's chain: degrid the model grid (nterms = 1) with the fused residual, then grid the residuals onto
+    two Taylor-weighted grids."""
+    wl = W.make_workload(W.small_config(5))
+    rp1, rp2 = ref.plan_for(wl, nterms=1), ref.plan_for(wl, nterms=2)
+    res_want = rp1.degrid(wl.uvw, wl.freq, wl.cf_index, wl.model_grid.astype(np.complex128), None, vis_in=wl.vis)
+    run1, run2 = run_for(B, wl, nterms=1), run_for(B, wl, nterms=2)
+    try:
+        res = run1.degrid(wl.model_grid, None, vis_in=wl.vis)
+        assert_close(res, res_want, "cfg5 residual")
+        want, want_sw = rp2.grid(wl.uvw, wl.freq, wl.cf_index, res, wl.wt, wl.tau)
+        got, sw = run2.grid(res, wl.wt, wl.tau)
+        assert_close(got, want, "cfg5 multi-term grid")
+        assert np.abs(sw - want_sw).max() <= 1e-6 * np.abs(want_sw).max()
+    finally:
+        run1.close()
+        run2.close()
+
+
+@pytest.mark.parametrize("ncorr,nterms,os_,supports,tile", [(1, 1, 4, [1, 3], 32), (3, 1, 2, [5, 35, 65], 32), (4, 2, 1, [9], 16),
+                                                            (2, 3, 3, [7, 67], 32), (1, 4, 8, [33, 31], 8), (2, 2, 4, [17, 45], 64)])
+def test_grid_and_degrid_random_tables(B, ref, ncorr, nterms, os_, supports, tile):
+    """Random complex (non-separable) kernels, supports across all gridder classes (<= 33, <= 65, > 65), odd
+    correlation / term counts, ragged point counts, points off the grid, accumulate-into semantics."""
+    rng = np.random.default_rng(1000 + ncorr * 10 + nterms)
+    nx, ny, n, nchan = 160, 144, 777, 3
+    ks = [(rng.standard_normal((S * os_, S * os_)) + 1j * rng.standard_normal((S * os_, S * os_))).astype(np.complex64) for S in supports]
+    sup = np.array(supports, np.int32)
+    off = np.concatenate([[0], np.cumsum([k.size for k in ks])[:-1]]).astype(np.int64)
+    data = np.concatenate([k.ravel() for k in ks])
+    uvw = np.stack([rng.uniform(-nx / 2 - 3, nx / 2 + 3, n), rng.uniform(-ny / 2 - 3, ny / 2 + 3, n), np.zeros(n)], 1)
+    freq = C_LIGHT * (1.0 + 0.02 * np.arange(nchan))
+    cfi = rng.integers(0, len(supports), (n, nchan)).astype(np.int32)
+    vis = (rng.standard_normal((n, nchan, ncorr)) + 1j * rng.standard_normal((n, nchan, ncorr))).astype(np.complex64)
+    wt = rng.uniform(0.5, 1, (n, nchan, ncorr)).astype(np.float32)
+    wt[rng.random((n, nchan, ncorr)) < 0.05] = 0.0           # flags as zero weight (R4)
+    tau = rng.uniform(-1, 1, (nchan, nterms)).astype(np.float32) if nterms > 1 else None
+    rp = ref.RefPlan(nx, ny, ncorr, nterms, os_, 0.97, -1.02, sup, off, data, tile=tile, sort_mode=1)
+    run = GpuRun(B, nx, ny, ncorr, nterms, os_, 0.97, -1.02, sup, off, data, uvw, freq, cfi, tile=tile, sort_mode=1)
+    try:
+        assert_bin_equal(run.export(), rp.bin(uvw, freq, cfi))
+        g0 = (rng.standard_normal((nterms, ncorr, ny, nx)) + 1j * rng.standard_normal((nterms, ncorr, ny, nx))).astype(np.complex64)
+        want, want_sw = rp.grid(uvw, freq, cfi, vis, wt, tau, grid=g0.astype(np.complex128))
+        for variant in (0, 1):
+            got, sw = run.grid(vis, wt, tau, variant=variant, grid0=g0)
+            assert_close(got, want, f"random table variant {variant}")
+            assert np.abs(sw - want_sw).max() <= 1e-6 * np.abs(want_sw).max()
+        gm = (rng.standard_normal((nterms, ncorr, ny, nx)) + 1j * rng.standard_normal((nterms, ncorr, ny, nx))).astype(np.complex64)
+        want_v = rp.degrid(uvw, freq, cfi, gm.astype(np.complex128), tau, vis_in=vis)
+        got_v = run.degrid(gm, tau, vis_in=vis)
+        assert_close(got_v, want_v, "random table degrid")
+        invalid = rp.bin(uvw, freq, cfi)["key"] == np.uint64(2 ** 64 - 1)
+        assert invalid.any()
+        assert np.array_equal(got_v.reshape(-1, ncorr)[invalid], vis.reshape(-1, ncorr)[invalid])   # V = 0 there
+    finally:
+        run.close()
+
+
+def test_empty_and_state_errors(B):
+    sup, off, data = np.array([3], np.int32), np.array([0], np.int64), np.ones(9, np.complex64)
+    plan = B.lra_plan_create(64, 64, 1, 1, 1, 1.0, 1.0, sup, off, data)
+    try:
+        g = torch.zeros((1, 1, 64, 64), dtype=torch.complex64, device="cuda")
+        with pytest.raises(B.LraError):
+            B.lra_grid(plan, g, torch.zeros(1, device="cuda"), None, g)          # before lra_bin: LRA_ESTATE
+        B.lra_bin(plan, torch.zeros((0, 3), dtype=torch.float64, device="cuda"), np.array([C_LIGHT]))
+        assert B.lra_bin_export(plan) == 0
+        B.lra_grid(plan, torch.zeros((0, 1, 1), dtype=torch.complex64, device="cuda"),
+                   torch.zeros((0, 1, 1), dtype=torch.float32, device="cuda"), None, g)
+        torch.cuda.synchronize()
+        assert not g.abs().any()
+        assert B.lra_launch_count(plan) >= 1
+    finally:
+        B.lra_plan_destroy(plan)
+
+
+def test_p4_exact_patch_in_fp32(B):
+    """Pin P4 on the GPU: a single unit visibility at a pixel centre reproduces the kernel samples exactly."""
+    S, os_, nx = 7, 20, 64
+    K = W.ps_kernel(S, os_)
+    h, c0 = 3, 3 * os_ + os_ // 2 - 1
+    run = GpuRun(B, nx, nx, 1, 1, os_, 1.0, 1.0, [S], [0], K.ravel(), np.array([[5.0 + 1.0 / os_, -9.0, 0.0]]), np.array([C_LIGHT]), None)
+    try:
+        g, sw = run.grid(np.ones((1, 1, 1), np.complex64), np.ones((1, 1, 1), np.float32))
+        X, Y = 32 + 5, 32 - 9
+        expect = K[c0 - h * os_:c0 + h * os_ + 1:os_, c0 - 1 - h * os_:c0 - 1 + h * os_ + 1:os_]
+        assert np.array_equal(g[0, 0, Y - h:Y + h + 1, X - h:X + h + 1], expect)
+        assert np.count_nonzero(g) == np.count_nonzero(expect) and sw[0, 0] == 1.0
+    finally:
+        run.close()
