@@ -1,0 +1,322 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the gridding / degridding hot path on B200.
+
+A "step" is one pass of the whole hot path over one batch of synthetic input:
+lra_bin (index + bucket sort) -> lra_grid (tap loop + tile flush + sum of weights) -> lra_degrid (model
+prediction with the fused residual).  Workload at N = 1: BASELINE.json configs[2], the VLA-like W-projection
+configuration the target is quoted on (40,435,200 visibility points x 2 correlations, 8192^2 grid, 128 w-planes,
+supports 9..65, oversampling 8).  With N > 1 ranks every rank runs the same-sized shard (weak scaling; payload
+seeded per rank) and the per-rank grids are summed with one NCCL all-reduce per step (accumulation of partial
+grids).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3] [--small]
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2508_17187_b200 import workloads as W  # noqa: E402
+
+FP32_PEAK_TFLOPS_NOMINAL = 148 * 128 * 2 * 1.965e9 / 1e12   # 148 SMs x 128 FP32 lanes x 2 flop x 1965 MHz
+METRIC = "visibility points per second through bin+grid+degrid"
+UNIT = "vis_points/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--small", action="store_true", help="reduced config (debugging only; not a bench value)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--grid-variant", type=int, default=0)
+    return ap.parse_args()
+
+
+def measured_peaks():
+    try:
+        return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.stop, self.t = index, [], threading.Event(), None
+
+    def _run(self):
+        while not self.stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits"],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([x.strip() for x in out.split(",")])
+            except Exception:
+                pass
+            self.stop.wait(0.2)
+
+    def __enter__(self):
+        self.t = threading.Thread(target=self._run, daemon=True)
+        self.t.start()
+        return self
+
+    def __exit__(self, *a):
+        self.stop.set()
+        self.t.join(timeout=6)
+
+    def summary(self):
+        sm, mx, reasons = [], 0.0, set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx = max(mx, float(r[1]))
+            except Exception:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx or None, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def make_workload(args, rank):
+    cfg = W.small_config(args.config) if args.small else W.full_config(args.config)
+    wl = W.make_workload(cfg, with_payload=False)
+    n = cfg.npoints * cfg.ncorr
+    # payload seeded per rank (weak scaling: every rank grids its own shard of the same shape)
+    wl.vis = W.complex_normal(cfg.cfg_id, 2 + 16 * rank, n).reshape(cfg.nrow, cfg.nchan, cfg.ncorr)
+    wl.wt = W.uniform_f32(cfg.cfg_id, 3 + 16 * rank, n, 0.5, 1.0).reshape(cfg.nrow, cfg.nchan, cfg.ncorr)
+    return wl
+
+
+def oracle_sample(wl, args, target_taps=6.0e9):
+    """The oracle as it stands (oracle/lra_ref.c, fp64, OpenMP row bands) on a bounded sample of the workload:
+    the first `nt` time samples (all baselines, channels, correlations), bin + grid + degrid.  Returns
+    (points/s, seconds, cores, sample description, grid taps/s)."""
+    from oracle import lra_ref as R
+    cfg = wl.cfg
+    per_time = max(1, wl.sum_s2() * cfg.ncorr * cfg.nterms // cfg.ntimes)          # grid taps per time sample
+    nt = int(max(1, min(cfg.ntimes, target_taps // (2 * per_time))))               # grid + degrid
+    rows = W.N_BL * nt if cfg.kind != "disk" else cfg.nrow
+    sl = slice(0, rows)
+    cfi = None if wl.cf_index is None else wl.cf_index[sl]
+    plan = R.plan_for(wl, sort_mode=R.SORT_TILE_CF)
+    cores = R.max_threads()
+    t0 = time.perf_counter()
+    plan.bin(wl.uvw[sl], wl.freq, cfi)
+    t1 = time.perf_counter()
+    grid, _ = plan.grid(wl.uvw[sl], wl.freq, cfi, wl.vis[sl], wl.wt[sl], wl.tau)
+    t2 = time.perf_counter()
+    plan.degrid(wl.uvw[sl], wl.freq, cfi, grid, wl.tau, vis_in=wl.vis[sl])
+    t3 = time.perf_counter()
+    npts = rows * cfg.nchan
+    taps = (wl.sum_s2() if cfi is None else int((np.bincount(cfi.ravel(), minlength=len(wl.cf.support)).astype(np.int64)
+                                                 * wl.cf.support.astype(np.int64) ** 2).sum())) * cfg.ncorr * cfg.nterms
+    desc = (f"first {nt} of {cfg.ntimes} time samples ({npts} points x {cfg.ncorr} corr), bin {t1 - t0:.2f}s + grid "
+            f"{t2 - t1:.2f}s + degrid {t3 - t2:.2f}s, fp64, {cores} OpenMP threads")
+    return npts / (t3 - t0), t3 - t0, cores, desc, taps / (t2 - t1)
+
+
+def run_reference(args):
+    """--impl reference: the oracle timed on the host cores on the same config / metric (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    wl = make_workload(args, 0)
+    vals, info = [], None
+    for i in range(args.warmup + args.steps):
+        v, secs, cores, desc, gt = oracle_sample(wl, args, target_taps=2.0e9)
+        if i >= args.warmup:
+            vals.append((v, secs))
+        info = (cores, desc, gt)
+    value = float(np.mean([v for v, _ in vals]))
+    ms = float(np.mean([s for _, s in vals]) * 1e3)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": {"workload": wl.cfg.name, "note": "each step is a bounded sample: " + info[1]},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": info[0], "kind": "oracle", "sample": info[1]},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2508_17187_b200 import binding as B
+
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    B.lib()
+    wl = make_workload(args, rank)
+    cfg = wl.cfg
+    stream = torch.cuda.current_stream()
+    plan = B.lra_plan_create(cfg.nx, cfg.ny, cfg.ncorr, cfg.nterms, cfg.oversampling, wl.scale_u, wl.scale_v, wl.cf.support,
+                             wl.cf.offset, wl.cf.data, tile=cfg.tile, sort_mode=B.LRA_SORT_TILE_CF, device=local,
+                             stream=stream.cuda_stream)
+    B.lra_set_variant(plan, args.grid_variant, 0)
+    # host buffers (pinned) and their device copies
+    h_uvw = torch.from_numpy(wl.uvw).pin_memory()
+    h_cfi = None if wl.cf_index is None else torch.from_numpy(wl.cf_index).pin_memory()
+    h_vis = torch.from_numpy(wl.vis).pin_memory()
+    h_wt = torch.from_numpy(wl.wt).pin_memory()
+    d_uvw, d_vis, d_wt = h_uvw.cuda(), h_vis.cuda(), h_wt.cuda()
+    d_cfi = None if h_cfi is None else h_cfi.cuda()
+    d_tau = None if wl.tau is None else torch.from_numpy(wl.tau).cuda()
+    grid = torch.zeros((cfg.nterms, cfg.ncorr, cfg.ny, cfg.nx), dtype=torch.complex64, device="cuda")
+    sumwt = torch.zeros((cfg.nterms, cfg.ncorr), dtype=torch.float64, device="cuda")
+    res = torch.empty_like(d_vis)
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    phase_ms = {"bin": [], "grid": [], "degrid": [], "allreduce": []}
+
+    def step(record):
+        e = [ev() for _ in range(5)]
+        grid.zero_()
+        sumwt.zero_()
+        e[0].record()
+        B.lra_bin(plan, d_uvw, wl.freq, d_cfi)
+        e[1].record()
+        B.lra_grid(plan, d_vis, d_wt, d_tau, grid, sumwt)
+        e[2].record()
+        if world > 1:
+            dist.all_reduce(torch.view_as_real(grid))
+            dist.all_reduce(sumwt)
+        e[3].record()
+        B.lra_degrid(plan, grid, d_tau, d_vis, res)
+        e[4].record()
+        if record:
+            phase_ev.append(e)
+
+    def sync_all():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    phase_ev = []
+    for _ in range(args.warmup):
+        step(False)
+    sync_all()
+    l0 = B.lra_launch_count(plan)
+    with ClockSampler(local) as clk:
+        t_start, t_end = ev(), ev()
+        sync_all()
+        t_start.record()
+        for _ in range(args.steps):
+            step(True)
+        t_end.record()
+        sync_all()
+    total_ms = t_start.elapsed_time(t_end)
+    launches = B.lra_launch_count(plan) - l0 + args.steps * 2      # + the two zero-fill kernels per step
+    for e in phase_ev:
+        phase_ms["bin"].append(e[0].elapsed_time(e[1]))
+        phase_ms["grid"].append(e[1].elapsed_time(e[2]))
+        phase_ms["allreduce"].append(e[2].elapsed_time(e[3]))
+        phase_ms["degrid"].append(e[3].elapsed_time(e[4]))
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    n_valid, sum_s2 = B.lra_tap_count(plan)
+    ms_per_step = total_ms / args.steps
+    value = cfg.npoints * world / (ms_per_step * 1e-3)
+
+    # ---- end to end through the C ABI with HOST buffers: H2D of the step's inputs + D2H of its results ----
+    e2e = None
+    if not args.no_e2e:
+        h_grid = torch.empty(grid.shape, dtype=torch.complex64).pin_memory()
+        h_res = torch.empty(res.shape, dtype=torch.complex64).pin_memory()
+        h_sw = torch.empty(sumwt.shape, dtype=torch.float64).pin_memory()
+
+        def e2e_step():
+            d_uvw.copy_(h_uvw, non_blocking=True)
+            if d_cfi is not None:
+                d_cfi.copy_(h_cfi, non_blocking=True)
+            d_vis.copy_(h_vis, non_blocking=True)
+            d_wt.copy_(h_wt, non_blocking=True)
+            step(False)
+            h_grid.copy_(grid, non_blocking=True)
+            h_res.copy_(res, non_blocking=True)
+            h_sw.copy_(sumwt, non_blocking=True)
+
+        e2e_step()
+        sync_all()
+        k = max(1, min(args.steps, 3))
+        t0 = time.perf_counter()
+        a, b = ev(), ev()
+        a.record()
+        for _ in range(k):
+            e2e_step()
+        b.record()
+        sync_all()
+        e_ms = max(a.elapsed_time(b), (time.perf_counter() - t0) * 1e3) / k
+        if world > 1:
+            t = torch.tensor([e_ms], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e_ms = float(t.item())
+        h2d = h_uvw.numel() * 8 + (0 if h_cfi is None else h_cfi.numel() * 4) + h_vis.numel() * 8 + h_wt.numel() * 4
+        d2h = h_grid.numel() * 8 + h_res.numel() * 8 + h_sw.numel() * 8
+        e2e = {"value": cfg.npoints * world / (e_ms * 1e-3), "unit": UNIT, "ms_per_step": e_ms,
+               "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)}
+
+    if rank == 0:
+        peaks = measured_peaks()
+        med = {k: float(np.median(v)) if v else 0.0 for k, v in phase_ms.items()}
+        ngrids = cfg.ncorr * cfg.nterms
+        grid_taps = sum_s2 * ngrids
+        grid_flops = grid_taps * 8.0
+        achieved = grid_flops / (med["grid"] * 1e-3) / 1e12
+        roofline = {"bound": "alu", "kernel": "lra_grid (tiled register-accumulating gridder, all launches of one call)",
+                    "achieved": achieved, "peak": FP32_PEAK_TFLOPS_NOMINAL, "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS_NOMINAL,
+                    "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 flop x 1965 MHz (MEASURED_PEAKS.json has no FP32 entry)",
+                    "traffic": None, "tap_updates_per_launch": grid_taps, "tap_updates_per_s": grid_taps / (med["grid"] * 1e-3),
+                    "degrid_tap_updates_per_s": grid_taps / (med["degrid"] * 1e-3) if med["degrid"] else None,
+                    "hbm_gbs_measured_peak": None if not peaks else peaks.get("hbm_gbs")}
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+                "data": "synthetic",
+                "config": {"workload": cfg.name, "points": cfg.npoints, "ncorr": cfg.ncorr, "nterms": cfg.nterms,
+                           "grid": [cfg.ny, cfg.nx], "n_cf": cfg.n_cf, "oversampling": cfg.oversampling, "n_valid": n_valid,
+                           "sum_S2": sum_s2, "l2": "inputs larger than L2 (vis+wt 0.97 GB, grid 1.07 GB per step)",
+                           "parallelism": f"dp{world}" if world > 1 else "single"},
+                "phase_ms_median": med, "grid_vis_points_per_s": n_valid / (med["grid"] * 1e-3),
+                "roofline": roofline, "clocks": clk.summary(), "gpu_launches": int(launches)}
+        if e2e:
+            line["e2e"] = e2e
+        if not args.no_cpu_baseline and world == 1:
+            v, secs, cores, desc, gt = oracle_sample(wl, args)
+            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
+                                    "grid_tap_updates_per_s": gt}
+        print(json.dumps(line))
+    B.lra_plan_destroy(plan)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    a = parse()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)
