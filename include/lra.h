@@ -123,6 +123,12 @@ int lra_tap_count(lra_plan* p, int64_t* n_valid, int64_t* sum_s2);
  * listed in DESIGN.md (1 = plain global-atomic gridder kept as the "before" profile). */
 int lra_set_variant(lra_plan* p, int32_t grid_variant, int32_t degrid_variant);
 
+/* Measurement aids (not on the hot path; synchronous).  lra_diag_fma_tflops: FP32 FMA throughput of `device`
+ * in TFLOP/s from an FMA-only kernel -- the compute term of the gridding roofline.
+ * lra_diag_l2_gbs: read bandwidth in GB/s of an `mbytes`-MiB buffer kept in L2 -- the bound on CF-slab traffic. */
+int lra_diag_fma_tflops(int device, double* tflops);
+int lra_diag_l2_gbs(int device, int mbytes, double* gbs);
+
 const char* lra_strerror(int code);
 /* cudaGetErrorString of the last failing CUDA call of this plan ("" if none). */
 const char* lra_last_cuda_error(const lra_plan* p);

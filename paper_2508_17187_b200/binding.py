@@ -55,6 +55,8 @@ def lib() -> C.CDLL:
         L.lra_launch_count.restype = i64
         L.lra_tap_count.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
         L.lra_set_variant.argtypes = [vp, i32, i32]
+        L.lra_diag_fma_tflops.argtypes = [i32, C.POINTER(C.c_double)]
+        L.lra_diag_l2_gbs.argtypes = [i32, i32, C.POINTER(C.c_double)]
         L.lra_strerror.argtypes = [C.c_int]
         L.lra_strerror.restype = C.c_char_p
         L.lra_last_cuda_error.argtypes = [vp]
@@ -64,7 +66,8 @@ def lib() -> C.CDLL:
 
 
 EXPORTED = ["lra_plan_create", "lra_plan_destroy", "lra_bin", "lra_bin_export", "lra_grid", "lra_degrid",
-            "lra_launch_count", "lra_tap_count", "lra_set_variant", "lra_strerror", "lra_last_cuda_error"]
+            "lra_launch_count", "lra_tap_count", "lra_set_variant", "lra_strerror", "lra_last_cuda_error",
+            "lra_diag_fma_tflops", "lra_diag_l2_gbs"]
 
 
 def _check(rc: int, plan=None):
@@ -150,6 +153,18 @@ def lra_tap_count(plan: int):
 
 def lra_set_variant(plan: int, grid_variant: int = 0, degrid_variant: int = 0):
     _check(lib().lra_set_variant(plan, grid_variant, degrid_variant), plan)
+
+
+def lra_diag_fma_tflops(device: int = 0) -> float:
+    v = C.c_double(0)
+    _check(lib().lra_diag_fma_tflops(device, C.byref(v)))
+    return float(v.value)
+
+
+def lra_diag_l2_gbs(device: int = 0, mbytes: int = 64) -> float:
+    v = C.c_double(0)
+    _check(lib().lra_diag_l2_gbs(device, mbytes, C.byref(v)))
+    return float(v.value)
 
 
 def lra_strerror(code: int) -> str:
