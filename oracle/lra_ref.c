@@ -41,6 +41,7 @@ typedef struct {
   const int32_t* cf_support;
   const int64_t* cf_offset;
   const float* cf_data;
+  int32_t tile_x; /* R5: uv tiles are tile_x wide (u) and tile tall (v); 0 => square, tile_x = tile */
 } lra_ref_desc;
 
 enum { LRA_REF_SORT_TILE = 0, LRA_REF_SORT_TILE_CF = 1 };
@@ -110,9 +111,9 @@ static inline const float* tap_ptr(const lra_ref_desc* d, const ref_point* q, in
 /* Step 7: sort key (R5). */
 static uint64_t sort_key(const lra_ref_desc* d, const ref_point* q) {
   if (!q->valid) return UINT64_MAX;
-  int32_t T = d->tile, os = d->oversampling;
-  uint64_t ntx = (uint64_t)((d->nx + T - 1) / T);
-  uint64_t tile_id = (uint64_t)(q->iy / T) * ntx + (uint64_t)(q->ix / T);
+  int32_t Ty = d->tile, Tx = d->tile_x > 0 ? d->tile_x : d->tile, os = d->oversampling;
+  uint64_t ntx = (uint64_t)((d->nx + Tx - 1) / Tx);
+  uint64_t tile_id = (uint64_t)(q->iy / Ty) * ntx + (uint64_t)(q->ix / Tx);
   if (d->sort_mode == LRA_REF_SORT_TILE) return tile_id;
   return ((tile_id * (uint64_t)d->n_cf + (uint64_t)q->cf) * (uint64_t)os + (uint64_t)(q->fy + os / 2)) * (uint64_t)os +
          (uint64_t)(q->fx + os / 2);
@@ -163,8 +164,8 @@ int lra_ref_bin(const lra_ref_desc* d, int64_t nrow, int32_t nchan, const double
   if (perm) for (int64_t i = 0; i < nv; ++i) perm[i] = kv[i].k;
   if (n_valid) *n_valid = nv;
   if (tile_start) {
-    int32_t T = d->tile;
-    int64_t ntiles = (int64_t)((d->nx + T - 1) / T) * ((d->ny + T - 1) / T);
+    int32_t Ty = d->tile, Tx = d->tile_x > 0 ? d->tile_x : d->tile;
+    int64_t ntiles = (int64_t)((d->nx + Tx - 1) / Tx) * ((d->ny + Ty - 1) / Ty);
     uint64_t per_tile = 1;
     if (d->sort_mode == LRA_REF_SORT_TILE_CF) per_tile = (uint64_t)d->n_cf * d->oversampling * d->oversampling;
     int64_t pos = 0;

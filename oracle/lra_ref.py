@@ -32,7 +32,8 @@ class _Desc(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("ncorr", C.c_int32), ("nterms", C.c_int32),
                 ("oversampling", C.c_int32), ("tile", C.c_int32), ("sort_mode", C.c_int32),
                 ("scale_u", C.c_double), ("scale_v", C.c_double), ("n_cf", C.c_int32),
-                ("cf_support", C.c_void_p), ("cf_offset", C.c_void_p), ("cf_data", C.c_void_p)]
+                ("cf_support", C.c_void_p), ("cf_offset", C.c_void_p), ("cf_data", C.c_void_p),
+                ("tile_x", C.c_int32)]
 
 
 _lib = None
@@ -57,18 +58,18 @@ class RefPlan:
     """Holds the descriptor (grid dims, CF table, oversampling) the oracle calls share."""
 
     def __init__(self, nx, ny, ncorr, nterms, oversampling, scale_u, scale_v, cf_support, cf_offset, cf_data,
-                 tile=32, sort_mode=SORT_TILE):
+                 tile=32, sort_mode=SORT_TILE, tile_x=0):
         self.cf_support = np.ascontiguousarray(cf_support, dtype=np.int32)
         self.cf_offset = np.ascontiguousarray(cf_offset, dtype=np.int64)
         self.cf_data = np.ascontiguousarray(cf_data, dtype=np.complex64)
         self.nx, self.ny, self.ncorr, self.nterms, self.os, self.tile = nx, ny, ncorr, nterms, oversampling, tile
+        self.tile_x = tile_x or tile      # R5: tiles are tile_x wide (u) by tile tall (v)
         self.d = _Desc(nx, ny, ncorr, nterms, oversampling, tile, sort_mode, float(scale_u), float(scale_v),
-                       len(self.cf_support), _p(self.cf_support), _p(self.cf_offset), _p(self.cf_data))
+                       len(self.cf_support), _p(self.cf_support), _p(self.cf_offset), _p(self.cf_data), tile_x)
 
     @property
     def ntiles(self):
-        T = self.tile
-        return ((self.nx + T - 1) // T) * ((self.ny + T - 1) // T)
+        return ((self.nx + self.tile_x - 1) // self.tile_x) * ((self.ny + self.tile - 1) // self.tile)
 
     def _geom(self, uvw, freq, cf_index):
         uvw = np.ascontiguousarray(uvw, dtype=np.float64)
@@ -144,8 +145,9 @@ class RefPlan:
         return out
 
 
-def plan_for(wl, nterms=None, sort_mode=SORT_TILE, tile=None) -> RefPlan:
+def plan_for(wl, nterms=None, sort_mode=SORT_TILE, tile=None, tile_x=0) -> RefPlan:
     """RefPlan for a ``workloads.Workload`` (argument marshalling only)."""
     c = wl.cfg
     return RefPlan(c.nx, c.ny, c.ncorr, c.nterms if nterms is None else nterms, c.oversampling, wl.scale_u,
-                   wl.scale_v, wl.cf.support, wl.cf.offset, wl.cf.data, tile=tile or c.tile, sort_mode=sort_mode)
+                   wl.scale_v, wl.cf.support, wl.cf.offset, wl.cf.data, tile=tile or c.tile, sort_mode=sort_mode,
+                   tile_x=tile_x)

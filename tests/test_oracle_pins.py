@@ -309,8 +309,8 @@ def test_p9_bin_exact_rational_cfg1(ref):
     assert nvalid == b["n_valid"] == n     # the 0.4 N disk keeps every footprint on the grid
 
 
-@pytest.mark.parametrize("mode", [0, 1])
-def test_p9_bin_structure(ref, mode):
+@pytest.mark.parametrize("mode,Tx,Ty", [(0, 32, 32), (1, 32, 32), (1, 8, 64), (0, 16, 8)])
+def test_p9_bin_structure(ref, mode, Tx, Ty):
     wl = W.make_workload(W.small_config(3))
     # push some points off the grid / to bad CFs / to NaN so that invalid handling is exercised
     uvw = wl.uvw.copy()
@@ -320,7 +320,7 @@ def test_p9_bin_structure(ref, mode):
     uvw[23, 1] = np.inf
     cfi[40, 1] = -1
     cfi[41, 2] = wl.cfg.n_cf
-    p = ref.plan_for(wl, sort_mode=mode)
+    p = ref.plan_for(wl, sort_mode=mode, tile=Ty, tile_x=Tx)      # R5: tiles Tx wide (u) by Ty tall (v)
     b = p.bin(uvw, wl.freq, cfi)
     n = wl.cfg.npoints
     key, perm, ts = b["key"], b["perm"], b["tile_start"]
@@ -334,9 +334,9 @@ def test_p9_bin_structure(ref, mode):
     same = np.diff(ks.astype(np.int64)) == 0
     assert (np.diff(perm.astype(np.int64))[same] > 0).all()                    # stable: equal keys ascending k
     # keys from the exported indices
-    T, os_ = 32, wl.cfg.oversampling
-    ntx = (wl.cfg.nx + T - 1) // T
-    tile = (b["iy"][valid] // T).astype(np.uint64) * np.uint64(ntx) + (b["ix"][valid] // T).astype(np.uint64)
+    os_ = wl.cfg.oversampling
+    ntx = (wl.cfg.nx + Tx - 1) // Tx
+    tile = (b["iy"][valid] // Ty).astype(np.uint64) * np.uint64(ntx) + (b["ix"][valid] // Tx).astype(np.uint64)
     if mode == 0:
         expect = tile
     else:
@@ -345,8 +345,8 @@ def test_p9_bin_structure(ref, mode):
             * np.uint64(os_) + (b["fx"][valid].astype(np.int64) + os_ // 2).astype(np.uint64)
     assert np.array_equal(key[valid], expect)
     # tile_start: searchsorted over tile ids along perm
-    tile_sorted = (b["iy"][perm] // T).astype(np.int64) * ntx + (b["ix"][perm] // T).astype(np.int64)
-    ntiles = ntx * ((wl.cfg.ny + T - 1) // T)
+    tile_sorted = (b["iy"][perm] // Ty).astype(np.int64) * ntx + (b["ix"][perm] // Tx).astype(np.int64)
+    ntiles = ntx * ((wl.cfg.ny + Ty - 1) // Ty)
     assert len(ts) == ntiles + 1
     assert np.array_equal(ts, np.searchsorted(tile_sorted, np.arange(ntiles + 1), side="left").astype(np.uint32))
     assert ts[-1] == b["n_valid"]
