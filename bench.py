@@ -174,7 +174,7 @@ def run_ours(args):
     cfg = wl.cfg
     stream = torch.cuda.current_stream()
     plan = B.lra_plan_create(cfg.nx, cfg.ny, cfg.ncorr, cfg.nterms, cfg.oversampling, wl.scale_u, wl.scale_v, wl.cf.support,
-                             wl.cf.offset, wl.cf.data, tile=cfg.tile, sort_mode=B.LRA_SORT_TILE_CF, device=local,
+                             wl.cf.offset, wl.cf.data, tile=cfg.tile, tile_x=cfg.tile_x, sort_mode=B.LRA_SORT_TILE_CF, device=local,
                              stream=stream.cuda_stream)
     B.lra_set_variant(plan, args.grid_variant, 0)
     # host buffers (pinned) and their device copies

@@ -50,7 +50,8 @@ typedef struct {
   int32_t nx, ny;         /* grid size in pixels; u along x (fastest), v along y; origin pixel (nx/2, ny/2) [R1] */
   int32_t ncorr, nterms;  /* grids per call = nterms*ncorr; 1 <= ncorr <= 4, 1 <= nterms <= 4                  */
   int32_t oversampling;   /* os >= 1: sub-pixel phases per pixel of the CF table [R3]                        */
-  int32_t tile;           /* T: uv-tile edge in pixels used by the bucket sort, power of two >= 8 (default 32)   */
+  int32_t tile;           /* uv-tile height (v) in pixels used by the bucket sort, power of two in [4, 1024];
+                             0 = the library default, strips 8 wide by 64 tall [R5]                              */
   int32_t sort_mode;      /* LRA_SORT_TILE | LRA_SORT_TILE_CF [R5]                                             */
   double scale_u, scale_v; /* pixels per wavelength along u and v; sign allowed [R1]                            */
   int32_t n_cf;           /* number of kernels in the CF table                                                 */
@@ -60,11 +61,12 @@ typedef struct {
                              row sits (m - c0)/os pixels from the kernel centre, c0 = h*os + (os-1-os/2) [R3]   */
   int32_t device;         /* CUDA device ordinal                                                               */
   void* stream;           /* cudaStream_t all work of this plan is enqueued on (NULL = legacy default stream)  */
+  int32_t tile_x;         /* uv-tile width (u) in pixels, power of two in [4, 1024]; 0 = square tiles (= tile)  */
 } lra_plan_desc;
 
 /* PreCompute: validates the descriptor, copies the CF table to the device and re-lays
- * every oversampled kernel into phase-major slabs [cf][fy][fx][S][S] so that the S*S taps one visibility
- * point needs are contiguous.  Synchronises the plan's stream before returning (the host table may be freed).
+ * every oversampled kernel into phase-major slabs [cf][fy][fx][S][tile_x + S - 1] (zero padded rows) so that
+ * the S*S taps one visibility point needs are one contiguous piece.  Synchronises the plan's stream before returning (the host table may be freed).
  * Errors: LRA_EINVAL, LRA_ENOMEM, LRA_ECUDA.  *out is NULL on failure. */
 int lra_plan_create(lra_plan** out, const lra_plan_desc* desc);
 
@@ -86,7 +88,7 @@ int lra_bin(lra_plan* p, int64_t nrow, int32_t nchan, const double* uvw_m, const
 /* Copies the bin result out for checking (all device pointers, each may be NULL to skip it):
  *   ix, iy int32 [npoints], fx, fy int8 [npoints], key uint64 [npoints]  (invalid point: ix = iy = -1,
  *   fx = fy = 0, key = 2^64-1); perm uint32 [npoints] (first n_valid entries meaningful);
- *   tile_start uint32 [ntiles+1], ntiles = ceil(nx/T)*ceil(ny/T); n_valid: HOST int64.
+ *   tile_start uint32 [ntiles+1], ntiles = ceil(nx/tile_x)*ceil(ny/tile); n_valid: HOST int64.
  * Synchronises the plan's stream.  Errors: LRA_ESTATE before lra_bin. */
 int lra_bin_export(lra_plan* p, int32_t* ix, int32_t* iy, int8_t* fx, int8_t* fy, uint64_t* key, uint32_t* perm,
                    uint32_t* tile_start, int64_t* n_valid);

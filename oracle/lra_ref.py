@@ -148,6 +148,8 @@ class RefPlan:
 def plan_for(wl, nterms=None, sort_mode=SORT_TILE, tile=None, tile_x=0) -> RefPlan:
     """RefPlan for a ``workloads.Workload`` (argument marshalling only)."""
     c = wl.cfg
+    if tile is None:
+        tile, tile_x = c.tile, tile_x or c.tile_x
     return RefPlan(c.nx, c.ny, c.ncorr, c.nterms if nterms is None else nterms, c.oversampling, wl.scale_u,
-                   wl.scale_v, wl.cf.support, wl.cf.offset, wl.cf.data, tile=tile or c.tile, sort_mode=sort_mode,
+                   wl.scale_v, wl.cf.support, wl.cf.offset, wl.cf.data, tile=tile, sort_mode=sort_mode,
                    tile_x=tile_x)

@@ -28,7 +28,7 @@ class lra_plan_desc(C.Structure):
                 ("oversampling", C.c_int32), ("tile", C.c_int32), ("sort_mode", C.c_int32),
                 ("scale_u", C.c_double), ("scale_v", C.c_double), ("n_cf", C.c_int32),
                 ("cf_support", C.c_void_p), ("cf_offset", C.c_void_p), ("cf_data", C.c_void_p),
-                ("device", C.c_int32), ("stream", C.c_void_p)]
+                ("device", C.c_int32), ("stream", C.c_void_p), ("tile_x", C.c_int32)]
 
 
 _lib = None
@@ -96,13 +96,14 @@ def _host(a: np.ndarray, dtype) -> np.ndarray:
 
 
 def lra_plan_create(nx, ny, ncorr, nterms, oversampling, scale_u, scale_v, cf_support, cf_offset, cf_data,
-                    tile=32, sort_mode=LRA_SORT_TILE_CF, device=0, stream=None) -> int:
-    """-> opaque plan handle (int).  cf_* are HOST numpy arrays (lra.h: lra_plan_desc)."""
+                    tile=0, sort_mode=LRA_SORT_TILE_CF, device=0, stream=None, tile_x=0) -> int:
+    """-> opaque plan handle (int).  cf_* are HOST numpy arrays (lra.h: lra_plan_desc).  tile = 0: the library's
+    default 8 x 64 strips; tile_x = 0 with tile != 0: square tiles."""
     sup = _host(cf_support, np.int32)
     off = _host(cf_offset, np.int64)
     dat = _host(cf_data, np.complex64)
     d = lra_plan_desc(nx, ny, ncorr, nterms, oversampling, tile, sort_mode, float(scale_u), float(scale_v), len(sup),
-                      sup.ctypes.data, off.ctypes.data, dat.ctypes.data, device, stream or 0)
+                      sup.ctypes.data, off.ctypes.data, dat.ctypes.data, device, stream or 0, tile_x)
     h = C.c_void_p()
     _check(lib().lra_plan_create(C.byref(h), C.byref(d)))
     return h.value

@@ -22,7 +22,7 @@ __device__ __forceinline__ bool lra_axis_index(double coord_m, double s, int n, 
 }
 
 struct lra_index_args {
-  int nx, ny, os, tile, ntx, ntiles, sort_mode, n_cf, nchan;
+  int nx, ny, os, tile_x, tile_y, ntx, ntiles, sort_mode, n_cf, nchan;
   long long npoints;
   unsigned long long invalid_sort_key;  // ntiles * per_tile: sorts after every valid key
 };
@@ -51,7 +51,7 @@ lra_index_kernel(lra_index_args a, const double* __restrict__ uvw, const double*
     }
     unsigned long long key = ~0ull, skey = a.invalid_sort_key;
     if (ok) {
-      unsigned long long tile_id = (unsigned long long)(iy / a.tile) * a.ntx + (unsigned long long)(ix / a.tile);
+      unsigned long long tile_id = (unsigned long long)(iy / a.tile_y) * a.ntx + (unsigned long long)(ix / a.tile_x);
       key = tile_id;
       if (a.sort_mode == LRA_SORT_TILE_CF)
         key = ((tile_id * a.n_cf + cf) * a.os + (fy + a.os / 2)) * a.os + (fx + a.os / 2);
@@ -189,25 +189,21 @@ lra_record_kernel(const uint32_t* __restrict__ perm, const unsigned long long* _
                   const int32_t* __restrict__ ix, const int32_t* __restrict__ iy, const int8_t* __restrict__ fx,
                   const int8_t* __restrict__ fy, const int32_t* __restrict__ cf_index,
                   const int32_t* __restrict__ cf_support, const int64_t* __restrict__ slab_off, int os,
-                  lra_rec* __restrict__ rec) {
+                  int tile_x, lra_rec* __restrict__ rec) {
   long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
   if (i >= (long long)counters[0]) return;
   uint32_t k = perm[i];
   int cf = cf_index ? cf_index[k] : 0;
   int S = cf_support[cf];
-  int stride = (S * S + 1) & ~1;
+  int stride = 2 * lra_plane_floats(S, tile_x);
   int phase = (fy[k] + os / 2) * os + (fx[k] + os / 2);
   long long off = slab_off[cf] + (long long)phase * stride;
   lra_rec r;
   r.x = (uint32_t)ix[k] | ((uint32_t)iy[k] << 16);
-  r.y = (uint32_t)(off >> 1);
+  r.y = (uint32_t)(off >> 2);
   r.z = k;
   r.w = (uint32_t)S | ((uint32_t)cf << 8);
   rec[i] = r;
-}
-
-void lra_scan_kernel_launch(lra_plan* p, uint32_t* a, long long m) {
-  lra_scan_kernel<<<1, 1024, 0, p->stream>>>(a, m);
 }
 
 template <typename T>
@@ -252,7 +248,7 @@ int lra_bin_impl(lra_plan* p, int64_t nrow, int32_t nchan, const double* uvw, co
   LRA_CUDA(p, cudaMemcpyAsync(p->d_su, su.data(), nchan * sizeof(double), cudaMemcpyHostToDevice, p->stream));
   LRA_CUDA(p, cudaMemcpyAsync(p->d_sv, sv.data(), nchan * sizeof(double), cudaMemcpyHostToDevice, p->stream));
   LRA_CUDA(p, cudaStreamSynchronize(p->stream));  // su / sv are stack-owned
-  LRA_CUDA(p, cudaMemsetAsync(p->counters, 0, 16 * sizeof(unsigned long long), p->stream));
+  LRA_CUDA(p, cudaMemsetAsync(p->counters, 0, 64 * sizeof(unsigned long long), p->stream));
 
   unsigned long long per_tile = 1;
   if (p->sort_mode == LRA_SORT_TILE_CF) per_tile = (unsigned long long)p->n_cf * p->os * p->os;
@@ -261,7 +257,7 @@ int lra_bin_impl(lra_plan* p, int64_t nrow, int32_t nchan, const double* uvw, co
   p->sorted_buf = 0;
   if (n > 0) {
     lra_index_args a;
-    a.nx = p->nx; a.ny = p->ny; a.os = p->os; a.tile = p->tile; a.ntx = p->ntx; a.ntiles = p->ntiles;
+    a.nx = p->nx; a.ny = p->ny; a.os = p->os; a.tile_x = p->tile_x; a.tile_y = p->tile; a.ntx = p->ntx; a.ntiles = p->ntiles;
     a.sort_mode = p->sort_mode; a.n_cf = p->n_cf; a.nchan = nchan; a.npoints = n; a.invalid_sort_key = invalid_key;
     int blocks = (int)((n + 255) / 256);
     lra_index_kernel<<<blocks, 256, 0, p->stream>>>(a, uvw, p->d_su, p->d_sv, cf_index, p->d_cf_support, p->ix, p->iy,
@@ -300,7 +296,7 @@ int lra_bin_impl(lra_plan* p, int64_t nrow, int32_t nchan, const double* uvw, co
                                                                              p->tile_start);
     LRA_LAUNCH_CHECK(p);
     lra_record_kernel<<<blocks, 256, 0, p->stream>>>(p->sval[cur], p->counters, p->ix, p->iy, p->fx, p->fy, cf_index,
-                                                     p->d_cf_support, p->d_slab_off, p->os, p->rec);
+                                                     p->d_cf_support, p->d_slab_off, p->os, p->tile_x, p->rec);
     LRA_LAUNCH_CHECK(p);
     if ((rc = lra_build_work(p))) return rc;
   } else {

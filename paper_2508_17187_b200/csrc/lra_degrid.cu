@@ -19,8 +19,8 @@ lra_degrid_init_kernel(const float2* __restrict__ vis_in, float2* __restrict__ v
 template <int NC>
 __global__ void __launch_bounds__(256)
 lra_degrid_warp_kernel(const lra_rec* __restrict__ rec, const unsigned long long* __restrict__ counters,
-                       const float2* __restrict__ slabs, const float2* __restrict__ grid, const float* __restrict__ tau,
-                       const float2* vis_in, float2* vis_out, int nchan, int nterms, int nx, int ny) {
+                       const float* __restrict__ slabs, const float2* __restrict__ grid, const float* __restrict__ tau,
+                       const float2* vis_in, float2* vis_out, int nchan, int nterms, int nx, int ny, int tile_x) {
   const long long n = (long long)counters[0];
   const size_t plane = (size_t)nx * ny;
   const int lane = threadIdx.x & 31;
@@ -29,7 +29,8 @@ lra_degrid_warp_kernel(const lra_rec* __restrict__ rec, const unsigned long long
   for (long long i = warp0; i < n; i += nwarps) {
     const lra_rec r = rec[i];
     const int ix = r.x & 0xffff, iy = r.x >> 16, S = r.w & 0xff, h = (S - 1) >> 1;
-    const float2* slab = slabs + ((size_t)r.y << 1);
+    const float* slab = slabs + ((size_t)r.y << 2);
+    const int pf = lra_plane_floats(S, tile_x);
     const unsigned k = r.z;
     const int c = (int)(k % (unsigned)nchan);
     float tw[4];
@@ -41,7 +42,8 @@ lra_degrid_warp_kernel(const lra_rec* __restrict__ rec, const unsigned long long
     const float2* g0 = grid + (size_t)(iy - h) * nx + (ix - h);
     for (int j = 0; j < S; ++j) {
       for (int ii = lane; ii < S; ii += 32) {
-        const float2 cf = slab[j * S + ii];
+        const int ti = lra_tap_index(S, tile_x, j, ii);
+        const float2 cf = make_float2(slab[ti], slab[pf + ti]);
         const float2* gp = g0 + (size_t)j * nx + ii;
 #pragma unroll
         for (int p = 0; p < NC; ++p) {
@@ -90,7 +92,7 @@ int lra_degrid_impl(lra_plan* p, const float2* grid, const float* tau, const flo
   const int blocks = p->sm_count * 8;
 #define LRA_DG(NC)                                                                                                  \
   lra_degrid_warp_kernel<NC><<<blocks, 256, 0, p->stream>>>(p->rec, p->counters, p->slabs, grid, tau, vis_in, vis_out, \
-                                                            p->nchan, p->nterms, p->nx, p->ny)
+                                                            p->nchan, p->nterms, p->nx, p->ny, p->tile_x)
   switch (p->ncorr) {
     case 1: LRA_DG(1); break;
     case 2: LRA_DG(2); break;

@@ -4,8 +4,8 @@
 //   lra_sumwt_kernel        : sum of weights, per-thread fp64 partials -> block tree -> one atomic per block
 //   lra_grid_atomic_kernel  : variant 1, one CTA per visibility point, every tap a global float atomic (the
 //                             "before" design kept for profiling and as a second implementation in the tests)
-//   lra_grid_tiled_kernel   : variant 0 (default), see the comment at the kernel
-#include "lra_internal.cuh"
+//   lra_grid_strip_kernel   : variant 0 (default), lra_grid_strip.cu
+#include "lra_pipe.cuh"
 
 #define LRA_MAXG 16  // nterms * ncorr <= 4 * 4
 
@@ -60,15 +60,17 @@ lra_sumwt_kernel(const lra_rec* __restrict__ rec, const unsigned long long* __re
 // red.global.add.f32.  No staging, no reuse: this is the design the tiled kernel is measured against.
 __global__ void __launch_bounds__(256)
 lra_grid_atomic_kernel(const lra_rec* __restrict__ rec, const unsigned long long* __restrict__ counters,
-                       const float2* __restrict__ slabs, const float2* __restrict__ vis, const float* __restrict__ wt,
+                       const float* __restrict__ slabs, const float2* __restrict__ vis, const float* __restrict__ wt,
                        const float* __restrict__ tau, int nchan, int ncorr, int nterms, int nx, int ny,
-                       float2* __restrict__ grid) {
+                       int tile_x, int tile_y, int only_fallback, float2* __restrict__ grid) {
   const long long n = (long long)counters[0];
   const size_t plane = (size_t)nx * ny;
   for (long long i = blockIdx.x; i < n; i += gridDim.x) {
     const lra_rec r = rec[i];
     const int ix = r.x & 0xffff, iy = r.x >> 16, S = r.w & 0xff, h = (S - 1) >> 1;
-    const float2* slab = slabs + ((size_t)r.y << 1);
+    if (only_fallback && lra_group_of(S, tile_x, tile_y) != LRA_NGROUP - 1) continue;   // the strip kernels did those
+    const float* slab = slabs + ((size_t)r.y << 2);
+    const int pf = lra_plane_floats(S, tile_x);
     const uint32_t k = r.z;
     const int c = (int)(k % (uint32_t)nchan);
     float2 val[LRA_MAXG];
@@ -86,7 +88,8 @@ lra_grid_atomic_kernel(const lra_rec* __restrict__ rec, const unsigned long long
       }
     for (int e = threadIdx.x; e < S * S; e += 256) {
       const int j = e / S, ii = e - j * S;
-      const float2 cf = slab[e];
+      const int ti = lra_tap_index(S, tile_x, j, ii);
+      const float2 cf = make_float2(slab[ti], slab[pf + ti]);
       const size_t pix = (size_t)(iy - h + j) * nx + (ix - h + ii);
 #pragma unroll
       for (int t = 0; t < 4; ++t)
@@ -102,8 +105,8 @@ lra_grid_atomic_kernel(const lra_rec* __restrict__ rec, const unsigned long long
   }
 }
 
-// defined in lra_grid_tiled.cu
-int lra_grid_tiled_launch(lra_plan* p, const float2* vis, const float* wt, const float* tau, float2* grid);
+// defined in lra_grid_strip.cu
+int lra_grid_strip_launch(lra_plan* p, const float2* vis, const float* wt, const float* tau, float2* grid);
 
 int lra_grid_impl(lra_plan* p, const float2* vis, const float* wt, const float* tau, float2* grid, double* sumwt) {
   if (p->npoints == 0) return LRA_OK;
@@ -112,11 +115,13 @@ int lra_grid_impl(lra_plan* p, const float2* vis, const float* wt, const float* 
                                                             p->nterms, sumwt);
     LRA_LAUNCH_CHECK(p);
   }
-  if (p->grid_variant == 1 || p->tile > 32) {  // the tiled kernel's regions are built for T <= 32
+  const bool all_atomic = p->grid_variant == 1;
+  if (all_atomic || p->n_items[LRA_NGROUP - 1] > 0) {  // regions that fit no strip group (or the "before" variant)
     lra_grid_atomic_kernel<<<p->sm_count * 16, 256, 0, p->stream>>>(p->rec, p->counters, p->slabs, vis, wt, tau,
-                                                                     p->nchan, p->ncorr, p->nterms, p->nx, p->ny, grid);
+                                                                     p->nchan, p->ncorr, p->nterms, p->nx, p->ny,
+                                                                     p->tile_x, p->tile, all_atomic ? 0 : 1, grid);
     LRA_LAUNCH_CHECK(p);
-    return LRA_OK;
+    if (all_atomic) return LRA_OK;
   }
-  return lra_grid_tiled_launch(p, vis, wt, tau, grid);
+  return lra_grid_strip_launch(p, vis, wt, tau, grid);
 }

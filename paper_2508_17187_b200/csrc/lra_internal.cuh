@@ -10,25 +10,27 @@
 
 // One sorted visibility point as the gridder / degridder consume it (16 bytes, one LDG.128).
 //   x: ix | iy << 16        (grid pixel of the footprint CENTRE; nx, ny <= 32768)
-//   y: slab element offset >> 1 (slabs are padded to an even number of complex64 => 16-byte aligned)
+//   y: slab offset in 16-byte units (float offset >> 2; every slab is 16-byte aligned)
 //   z: k = r*nchan + c      (index of the point in the caller's arrays)
 //   w: S | cf << 8          (support in pixels, kernel number)
 typedef uint4 lra_rec;
 
+#define LRA_NGROUP 5   // kernel configurations of the strip gridder / degridder; the last one is the fallback
+
 struct lra_plan {
   // ---- descriptor (host copies) ----
-  int32_t nx, ny, ncorr, nterms, os, tile, sort_mode, n_cf;
+  int32_t nx, ny, ncorr, nterms, os, tile, tile_x, sort_mode, n_cf;   // tiles are tile_x wide (u) by tile tall (v)
   double scale_u, scale_v;
   int device;
   cudaStream_t stream;
   std::vector<int32_t> cf_support;
-  std::vector<int64_t> slab_off;   // element offset of slab (cf, 0, 0) in `slabs`
-  std::vector<int32_t> slab_stride;  // elements per slab of kernel cf: S*S rounded up to even
+  std::vector<int64_t> slab_off;   // float offset of slab (cf, 0, 0) in `slabs`
+  std::vector<int32_t> slab_stride;  // floats per slab of kernel cf: 2 * lra_plane_floats(S, tile_x)
   int32_t max_support;
   int32_t ntx, nty, ntiles;
   // ---- device: CF store ----
-  float2* slabs;            // [cf][fy][fx][S][S] phase-major, each slab 16-byte aligned
-  int64_t slab_elems;
+  float* slabs;             // [cf][fy][fx] phase-major PLANAR slabs, see lra_plane_floats()
+  int64_t slab_elems;       // total floats
   int32_t* d_cf_support;    // [n_cf]
   int64_t* d_slab_off;      // [n_cf]
   // ---- device: bin state ----
@@ -46,19 +48,37 @@ struct lra_plan {
   int64_t hist_capacity;
   uint32_t* tile_start;     // [ntiles + 1]
   lra_rec* rec;             // [npoints] sorted records (first n_valid meaningful)
-  unsigned long long* counters;  // [0] n_valid, [1] sum S^2, [2..] scratch
+  unsigned long long* counters;  // see lra_pipe.cuh
   double *d_su, *d_sv;      // per-channel scale tables
   int32_t su_capacity;
-  // ---- gridder work list ----
-  void* work;               // uint4 work items for the tiled gridder
-  uint32_t* item_off;       // [ntiles + 1] first work item of every tile
+  // ---- work lists of the strip kernels (lra_work.cu; geometry only, rebuilt by every lra_bin) ----
+  uint4* work;              // items of all groups, grouped by group
   int64_t work_capacity;
+  uint4* stage_hdr;         // stage headers of all groups, grouped by group; an item's stages are consecutive
+  int64_t stage_capacity;
+  uint32_t* pw;             // [npoints][16] per-point, per-consumer-warp words (tap offset | step mask << 16)
+  int64_t pw_capacity;      // points
+  float* prep;              // gridder: wt*tau*V of every sorted point, FFMA2 operand form; degridder: sorted results
+  int64_t prep_capacity;    // floats
+  int64_t n_items[8], item_off[8];     // items per group and first item of every group in `work`
+  int64_t n_stages[8], stage_off[8];   // stages per group and first stage of every group in `stage_hdr`
   // ---- misc ----
   int32_t grid_variant, degrid_variant;
   int64_t launches;
   cudaError_t last_err;
   int sm_count;
 };
+
+// Slab layout (one slab = the S*S taps of one kernel at one sub-pixel phase, what one visibility point needs).
+// A strip kernel works on a REGION of RX = S + tile_x - 1 columns (tile + halo) whose pixels are numbered
+// e = y*RX + x, and it reads the tap that a point with footprint origin (ox, oy) puts on pixel e at the linear
+// slab index e - (oy*RX + ox).  So a slab is stored with the region's pitch: two planes (real parts, then
+// imaginary parts) of PF = lra_plane_floats(S, tile_x) floats, tap (j, i), 0 <= j, i < S, at float j*RX + i, and
+// EVERY other float of the plane zero: the RX - S pad floats that end each row and the >= 64 floats that follow
+// the last row.  A lane that looks at a pixel outside the footprint therefore reads a zero instead of branching.
+// PF is a multiple of 4 (16 bytes) so that one TMA bulk copy moves a plane.
+__host__ __device__ inline int lra_plane_floats(int S, int tile_x) { return (S * (S + tile_x - 1) + 64 + 3) & ~3; }
+__host__ __device__ inline int lra_tap_index(int S, int tile_x, int j, int i) { return j * (S + tile_x - 1) + i; }
 
 #define LRA_CUDA(p, call)                         \
   do {                                            \
@@ -75,10 +95,9 @@ struct lra_plan {
     LRA_CUDA(p, cudaGetLastError());              \
   } while (0)
 
-// implemented in lra_grid.cu / lra_degrid.cu / lra_bin.cu
+// implemented in lra_grid.cu / lra_degrid.cu / lra_bin.cu / lra_work.cu
 int lra_grid_impl(lra_plan* p, const float2* vis, const float* wt, const float* tau, float2* grid, double* sumwt);
 int lra_degrid_impl(lra_plan* p, const float2* grid, const float* tau, const float2* vis_in, float2* vis_out);
 int lra_build_work(lra_plan* p);
-void lra_scan_kernel_launch(lra_plan* p, uint32_t* a, long long m);
 int lra_bin_impl(lra_plan* p, int64_t nrow, int32_t nchan, const double* uvw, const double* freq_host,
                  const int32_t* cf_index);

@@ -5,23 +5,32 @@
 
 #include "lra_internal.cuh"
 
-// Re-lay one oversampled kernel into phase-major slabs (reading R3):
-//   slab(fyi, fxi)[j + h][i + h] = K[(j*os - fy) + c0][(i*os - fx) + c0],  fy = fyi - os/2, c0 = h*os + (os-1-os/2)
-// One thread per slab element; padding elements (slab_stride > S*S) are zero-filled.
-__global__ void lra_relayout_kernel(const float2* __restrict__ K, float2* __restrict__ slab, int S, int os,
-                                    int slab_stride) {
+// Re-lay one oversampled kernel into phase-major planar slabs (reading R3; layout in
+// lra_internal.cuh):  tap (j + h, i + h) of slab (fyi, fxi) = K[(j*os - fy) + c0][(i*os - fx) + c0],
+//   fy = fyi - os/2, c0 = h*os + (os-1-os/2).
+// One thread per output float; the padding floats are zero-filled.
+__global__ void lra_relayout_kernel(const float2* __restrict__ K, float* __restrict__ slab, int S, int os,
+                                    int slab_stride, int tile_x) {
   const int h = (S - 1) / 2;
+  const int rx = S + tile_x - 1;
   const int c0 = h * os + (os - 1 - os / 2);
+  const int pf = slab_stride >> 1;
   const int64_t n = (int64_t)os * os * slab_stride;
   const int64_t ld = (int64_t)S * os;
   for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
     int phase = (int)(e / slab_stride), t = (int)(e % slab_stride);
-    float2 v = make_float2(0.f, 0.f);
-    if (t < S * S) {
-      int fyi = phase / os, fxi = phase % os;
-      int j = t / S - h, i = t % S - h;
-      int row = j * os - (fyi - os / 2) + c0, col = i * os - (fxi - os / 2) + c0;
-      v = K[row * ld + col];
+    const int im = t >= pf;
+    if (im) t -= pf;
+    float v = 0.f;
+    {
+      int jj = t / rx, ii = t - jj * rx;
+      if (jj < S && ii < S) {
+        int fyi = phase / os, fxi = phase % os;
+        int j = jj - h, i = ii - h;
+        int row = j * os - (fyi - os / 2) + c0, col = i * os - (fxi - os / 2) + c0;
+        float2 k = K[row * ld + col];
+        v = im ? k.y : k.x;
+      }
     }
     slab[e] = v;
   }
@@ -35,8 +44,10 @@ extern "C" int lra_plan_create(lra_plan** out, const lra_plan_desc* d) {
   if (!d || d->nx < 1 || d->ny < 1 || d->nx > 32768 || d->ny > 32768) return LRA_EINVAL;
   if (d->ncorr < 1 || d->ncorr > 4 || d->nterms < 1 || d->nterms > 4) return LRA_EINVAL;
   if (d->oversampling < 1 || d->oversampling > 64) return LRA_EINVAL;
-  int tile = d->tile == 0 ? 32 : d->tile;
-  if (!is_pow2(tile) || tile < 8 || tile > 1024) return LRA_EINVAL;
+  // tile = 0: the library's default strip, 8 wide (u) by 64 tall (v); tile_x = 0 with tile != 0: square tiles
+  int tile = d->tile == 0 ? 64 : d->tile;
+  int tile_x = d->tile_x == 0 ? (d->tile == 0 ? 8 : tile) : d->tile_x;
+  if (!is_pow2(tile) || tile < 4 || tile > 1024 || !is_pow2(tile_x) || tile_x < 4 || tile_x > 1024) return LRA_EINVAL;
   if (d->sort_mode != LRA_SORT_TILE && d->sort_mode != LRA_SORT_TILE_CF) return LRA_EINVAL;
   if (d->n_cf < 1 || d->n_cf > (1 << 24) || !d->cf_support || !d->cf_offset || !d->cf_data) return LRA_EINVAL;
   if (!(d->scale_u == d->scale_u) || !(d->scale_v == d->scale_v)) return LRA_EINVAL;
@@ -47,10 +58,10 @@ extern "C" int lra_plan_create(lra_plan** out, const lra_plan_desc* d) {
   lra_plan* p = new (std::nothrow) lra_plan();
   if (!p) return LRA_ENOMEM;
   p->nx = d->nx; p->ny = d->ny; p->ncorr = d->ncorr; p->nterms = d->nterms; p->os = d->oversampling;
-  p->tile = tile; p->sort_mode = d->sort_mode; p->n_cf = d->n_cf;
+  p->tile = tile; p->tile_x = tile_x; p->sort_mode = d->sort_mode; p->n_cf = d->n_cf;
   p->scale_u = d->scale_u; p->scale_v = d->scale_v;
   p->device = d->device; p->stream = (cudaStream_t)d->stream;
-  p->ntx = (p->nx + tile - 1) / tile; p->nty = (p->ny + tile - 1) / tile; p->ntiles = p->ntx * p->nty;
+  p->ntx = (p->nx + tile_x - 1) / tile_x; p->nty = (p->ny + tile - 1) / tile; p->ntiles = p->ntx * p->nty;
   p->last_err = cudaSuccess;
   p->cf_support.assign(d->cf_support, d->cf_support + d->n_cf);
   p->slab_off.resize(d->n_cf);
@@ -59,14 +70,14 @@ extern "C" int lra_plan_create(lra_plan** out, const lra_plan_desc* d) {
   p->max_support = 1;
   for (int c = 0; c < d->n_cf; ++c) {
     int S = p->cf_support[c];
-    p->slab_stride[c] = (S * S + 1) & ~1;
+    p->slab_stride[c] = 2 * lra_plane_floats(S, tile_x);
     p->slab_off[c] = total;
     total += (int64_t)p->os * p->os * p->slab_stride[c];
     int64_t n_in = (int64_t)S * p->os * S * p->os;
     if (n_in > max_in) max_in = n_in;
     if (S > p->max_support) p->max_support = S;
   }
-  if ((total >> 1) >= (int64_t)1 << 32) { delete p; return LRA_EINVAL; }
+  if ((total >> 2) >= (int64_t)1 << 32) { delete p; return LRA_EINVAL; }
   p->slab_elems = total;
 
   float2* staging = nullptr;
@@ -75,10 +86,11 @@ extern "C" int lra_plan_create(lra_plan** out, const lra_plan_desc* d) {
     return fail(e__ == cudaErrorMemoryAllocation ? LRA_ENOMEM : LRA_ECUDA); } } while (0)
   CK(cudaSetDevice(p->device));
   CK(cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, p->device));
-  CK(cudaMalloc(&p->slabs, (size_t)total * sizeof(float2)));
+  CK(cudaMalloc(&p->slabs, (size_t)total * sizeof(float)));
   CK(cudaMalloc(&p->d_cf_support, (size_t)d->n_cf * sizeof(int32_t)));
   CK(cudaMalloc(&p->d_slab_off, (size_t)d->n_cf * sizeof(int64_t)));
-  CK(cudaMalloc(&p->counters, 64 * sizeof(unsigned long long)));
+  CK(cudaMalloc(&p->counters, 128 * sizeof(unsigned long long)));
+  CK(cudaMemsetAsync(p->counters, 0, 128 * sizeof(unsigned long long), p->stream));
   CK(cudaMalloc(&p->tile_start, (size_t)(p->ntiles + 1) * sizeof(uint32_t)));
   CK(cudaMemcpyAsync(p->d_cf_support, p->cf_support.data(), (size_t)d->n_cf * sizeof(int32_t), cudaMemcpyHostToDevice, p->stream));
   CK(cudaMemcpyAsync(p->d_slab_off, p->slab_off.data(), (size_t)d->n_cf * sizeof(int64_t), cudaMemcpyHostToDevice, p->stream));
@@ -93,7 +105,7 @@ extern "C" int lra_plan_create(lra_plan** out, const lra_plan_desc* d) {
     int64_t n_out = (int64_t)p->os * p->os * p->slab_stride[c];
     int blocks = (int)((n_out + 255) / 256);
     if (blocks > 4096) blocks = 4096;
-    lra_relayout_kernel<<<blocks, 256, 0, p->stream>>>(staging, p->slabs + p->slab_off[c], S, p->os, p->slab_stride[c]);
+    lra_relayout_kernel<<<blocks, 256, 0, p->stream>>>(staging, p->slabs + p->slab_off[c], S, p->os, p->slab_stride[c], tile_x);
     p->launches++;
     CK(cudaGetLastError());
   }
@@ -110,7 +122,7 @@ extern "C" int lra_plan_destroy(lra_plan* p) {
   cudaSetDevice(p->device);
   cudaStreamSynchronize(p->stream);
   void* ptrs[] = {p->slabs, p->d_cf_support, p->d_slab_off, p->ix, p->iy, p->fx, p->fy, p->key, p->skey[0], p->skey[1],
-                  p->sval[0], p->sval[1], p->hist, p->tile_start, p->rec, p->counters, p->d_su, p->d_sv, p->work, p->item_off};
+                  p->sval[0], p->sval[1], p->hist, p->tile_start, p->rec, p->counters, p->d_su, p->d_sv, p->work, p->stage_hdr, p->pw, p->prep};
   for (void* q : ptrs)
     if (q) cudaFree(q);
   delete p;

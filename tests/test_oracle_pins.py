@@ -291,7 +291,7 @@ def test_p8_partition_and_permutation(ref):
 # ---------------------------------------------------------------------------------------------------
 def test_p9_bin_exact_rational_cfg1(ref):
     wl = W.make_workload(W.full_config(1))
-    p = ref.plan_for(wl)
+    p = ref.plan_for(wl, tile=32)
     b = p.bin(wl.uvw, wl.freq, None)
     n = wl.cfg.npoints
     h = 3

@@ -10,6 +10,7 @@ pytestmark = pytest.mark.gpu
 
 torch = pytest.importorskip("torch")
 C_LIGHT = 299792458.0
+TILE = (8, 64)      # (tile_x, tile): the library's default strips, spelled out so that the oracle gets the same
 
 
 @pytest.fixture(scope="module")
@@ -28,12 +29,15 @@ def dev(a):
 class GpuRun:
     """One plan + bin on the GPU for a Workload-like bundle of numpy inputs."""
 
-    def __init__(self, B, nx, ny, ncorr, nterms, os_, su, sv, sup, off, data, uvw, freq, cf_index, tile=32, sort_mode=1):
+    def __init__(self, B, nx, ny, ncorr, nterms, os_, su, sv, sup, off, data, uvw, freq, cf_index, tile=TILE[1], sort_mode=1,
+                 tile_x=TILE[0]):
         self.B = B
         self.shape = (nterms, ncorr, ny, nx)
-        self.plan = B.lra_plan_create(nx, ny, ncorr, nterms, os_, su, sv, sup, off, data, tile=tile, sort_mode=sort_mode)
+        self.plan = B.lra_plan_create(nx, ny, ncorr, nterms, os_, su, sv, sup, off, data, tile=tile, sort_mode=sort_mode,
+                                      tile_x=tile_x)
         self.nrow, self.nchan, self.ncorr = len(uvw), len(freq), ncorr
-        self.ntiles = ((nx + tile - 1) // tile) * ((ny + tile - 1) // tile)
+        tile_x = tile_x or tile
+        self.ntiles = ((nx + tile_x - 1) // tile_x) * ((ny + tile - 1) // tile)
         self.uvw, self.cfi = dev(uvw), dev(cf_index)
         B.lra_bin(self.plan, self.uvw, freq, self.cfi)
 
@@ -69,10 +73,15 @@ class GpuRun:
         self.B.lra_plan_destroy(self.plan)
 
 
-def run_for(B, wl, nterms=None, sort_mode=1, tile=32):
+def run_for(B, wl, nterms=None, sort_mode=1, tile=TILE[1], tile_x=TILE[0]):
     c = wl.cfg
     return GpuRun(B, c.nx, c.ny, c.ncorr, c.nterms if nterms is None else nterms, c.oversampling, wl.scale_u, wl.scale_v,
-                  wl.cf.support, wl.cf.offset, wl.cf.data, wl.uvw, wl.freq, wl.cf_index, tile=tile, sort_mode=sort_mode)
+                  wl.cf.support, wl.cf.offset, wl.cf.data, wl.uvw, wl.freq, wl.cf_index, tile=tile, sort_mode=sort_mode,
+                  tile_x=tile_x)
+
+
+def ref_for(ref, wl, nterms=None, sort_mode=1, tile=TILE[1], tile_x=TILE[0]):
+    return ref.plan_for(wl, nterms=nterms, sort_mode=sort_mode, tile=tile, tile_x=tile_x)
 
 
 def assert_close(got, want, what):
@@ -99,7 +108,7 @@ def test_bin_bit_exact(B, ref, n, mode):
     wl = W.make_workload(W.small_config(n))
     run = run_for(B, wl, sort_mode=mode)
     try:
-        assert_bin_equal(run.export(), ref.plan_for(wl, sort_mode=mode).bin(wl.uvw, wl.freq, wl.cf_index))
+        assert_bin_equal(run.export(), ref_for(ref, wl, sort_mode=mode).bin(wl.uvw, wl.freq, wl.cf_index))
     finally:
         run.close()
 
@@ -113,13 +122,13 @@ def test_bin_invalid_points_and_small_tile(B, ref):
     uvw[29, 0] = 1e300
     cfi[40, 1] = -1
     cfi[41, 2] = wl.cfg.n_cf
-    for tile, mode in ((8, 1), (16, 0), (64, 1)):
+    for tile, tile_x, mode in ((8, 0, 1), (16, 0, 0), (64, 0, 1), (32, 4, 1), (8, 128, 0)):
         c = wl.cfg
         run = GpuRun(B, c.nx, c.ny, c.ncorr, 1, c.oversampling, wl.scale_u, -wl.scale_v, wl.cf.support, wl.cf.offset,
-                     wl.cf.data, uvw, wl.freq, cfi, tile=tile, sort_mode=mode)
+                     wl.cf.data, uvw, wl.freq, cfi, tile=tile, sort_mode=mode, tile_x=tile_x)
         try:
             r = ref.RefPlan(c.nx, c.ny, c.ncorr, 1, c.oversampling, wl.scale_u, -wl.scale_v, wl.cf.support, wl.cf.offset,
-                            wl.cf.data, tile=tile, sort_mode=mode)
+                            wl.cf.data, tile=tile, sort_mode=mode, tile_x=tile_x)
             want = r.bin(uvw, wl.freq, cfi)
             assert want["n_valid"] < c.npoints
             assert_bin_equal(run.export(), want)
@@ -130,7 +139,7 @@ def test_bin_invalid_points_and_small_tile(B, ref):
 @pytest.mark.parametrize("n", [1, 2, 3, 4, 5])
 def test_grid_parity_small_configs(B, ref, n):
     wl = W.make_workload(W.small_config(n))
-    rp = ref.plan_for(wl)
+    rp = ref_for(ref, wl)
     want, want_sw = rp.grid(wl.uvw, wl.freq, wl.cf_index, wl.vis, wl.wt, wl.tau)
     run = run_for(B, wl)
     try:
@@ -153,7 +162,7 @@ def test_degrid_parity_small_configs(B, ref, n):
         g = wl.model_grid
     else:
         g = (rng.standard_normal((c.nterms, c.ncorr, c.ny, c.nx)) + 1j * rng.standard_normal((c.nterms, c.ncorr, c.ny, c.nx))).astype(np.complex64)
-    rp = ref.plan_for(wl)
+    rp = ref_for(ref, wl)
     run = run_for(B, wl)
     try:
         want = rp.degrid(wl.uvw, wl.freq, wl.cf_index, g.astype(np.complex128), wl.tau)
@@ -168,7 +177,7 @@ def test_cfg5_pipeline_degrid_then_multiterm_grid(B, ref):
     """Config 5's chain: degrid the model grid (nterms = 1) with the fused residual, then grid the residuals onto
     two Taylor-weighted grids."""
     wl = W.make_workload(W.small_config(5))
-    rp1, rp2 = ref.plan_for(wl, nterms=1), ref.plan_for(wl, nterms=2)
+    rp1, rp2 = ref_for(ref, wl, nterms=1), ref_for(ref, wl, nterms=2)
     res_want = rp1.degrid(wl.uvw, wl.freq, wl.cf_index, wl.model_grid.astype(np.complex128), None, vis_in=wl.vis)
     run1, run2 = run_for(B, wl, nterms=1), run_for(B, wl, nterms=2)
     try:
@@ -183,11 +192,14 @@ def test_cfg5_pipeline_degrid_then_multiterm_grid(B, ref):
         run2.close()
 
 
-@pytest.mark.parametrize("ncorr,nterms,os_,supports,tile", [(1, 1, 4, [1, 3], 32), (3, 1, 2, [5, 35, 65], 32), (4, 2, 1, [9], 16),
-                                                            (2, 3, 3, [7, 67], 32), (1, 4, 8, [33, 31], 8), (2, 2, 4, [17, 45], 64)])
-def test_grid_and_degrid_random_tables(B, ref, ncorr, nterms, os_, supports, tile):
-    """Random complex (non-separable) kernels, supports across all gridder classes (<= 33, <= 65, > 65), odd
-    correlation / term counts, ragged point counts, points off the grid, accumulate-into semantics."""
+@pytest.mark.parametrize("ncorr,nterms,os_,supports,tile,tile_x", [
+    (1, 1, 4, [1, 3], 64, 8), (3, 1, 2, [5, 35, 65], 64, 8), (4, 2, 1, [9], 16, 0), (2, 3, 3, [7, 67], 64, 8),
+    (1, 4, 8, [33, 31], 8, 0), (2, 2, 4, [17, 45], 64, 0), (2, 1, 2, [19, 53, 55], 64, 8), (2, 1, 2, [11, 29, 47], 32, 4),
+    (1, 2, 1, [3, 21], 4, 64)])
+def test_grid_and_degrid_random_tables(B, ref, ncorr, nterms, os_, supports, tile, tile_x):
+    """Random complex (non-separable) kernels, supports across all groups of the strip kernels (regions of up to
+    2048, 4096, 7168, 9216 pixels and the global-atomic fallback beyond), strips and square tiles, odd correlation /
+    term counts, ragged point counts, points off the grid, accumulate-into semantics."""
     rng = np.random.default_rng(1000 + ncorr * 10 + nterms)
     nx, ny, n, nchan = 160, 144, 777, 3
     ks = [(rng.standard_normal((S * os_, S * os_)) + 1j * rng.standard_normal((S * os_, S * os_))).astype(np.complex64) for S in supports]
@@ -201,8 +213,8 @@ def test_grid_and_degrid_random_tables(B, ref, ncorr, nterms, os_, supports, til
     wt = rng.uniform(0.5, 1, (n, nchan, ncorr)).astype(np.float32)
     wt[rng.random((n, nchan, ncorr)) < 0.05] = 0.0           # flags as zero weight (R4)
     tau = rng.uniform(-1, 1, (nchan, nterms)).astype(np.float32) if nterms > 1 else None
-    rp = ref.RefPlan(nx, ny, ncorr, nterms, os_, 0.97, -1.02, sup, off, data, tile=tile, sort_mode=1)
-    run = GpuRun(B, nx, ny, ncorr, nterms, os_, 0.97, -1.02, sup, off, data, uvw, freq, cfi, tile=tile, sort_mode=1)
+    rp = ref.RefPlan(nx, ny, ncorr, nterms, os_, 0.97, -1.02, sup, off, data, tile=tile, sort_mode=1, tile_x=tile_x)
+    run = GpuRun(B, nx, ny, ncorr, nterms, os_, 0.97, -1.02, sup, off, data, uvw, freq, cfi, tile=tile, sort_mode=1, tile_x=tile_x)
     try:
         assert_bin_equal(run.export(), rp.bin(uvw, freq, cfi))
         g0 = (rng.standard_normal((nterms, ncorr, ny, nx)) + 1j * rng.standard_normal((nterms, ncorr, ny, nx))).astype(np.complex64)
