@@ -14,6 +14,7 @@ grids, PAPER.md:347).
 from __future__ import annotations
 
 import argparse
+import dataclasses
 import json
 import os
 import subprocess
@@ -44,6 +45,8 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--grid-variant", type=int, default=0)
+    ap.add_argument("--tile", type=int, default=0, help="uv-tile height (0 = the config's, i.e. the library default)")
+    ap.add_argument("--tile-x", type=int, default=0, help="uv-tile width (with --tile)")
     return ap.parse_args()
 
 
@@ -99,6 +102,8 @@ class ClockSampler:
 
 def make_workload(args, rank):
     cfg = W.small_config(args.config) if args.small else W.full_config(args.config)
+    if args.tile:
+        cfg = dataclasses.replace(cfg, tile=args.tile, tile_x=args.tile_x or args.tile)
     wl = W.make_workload(cfg, with_payload=False)
     n = cfg.npoints * cfg.ncorr
     # payload seeded per rank (weak scaling: every rank grids its own shard of the same shape)

@@ -51,7 +51,7 @@ typedef struct {
   int32_t ncorr, nterms;  /* grids per call = nterms*ncorr; 1 <= ncorr <= 4, 1 <= nterms <= 4                  */
   int32_t oversampling;   /* os >= 1: sub-pixel phases per pixel of the CF table [R3]                        */
   int32_t tile;           /* uv-tile height (v) in pixels used by the bucket sort, power of two in [4, 1024];
-                             0 = the library default, strips 8 wide by 64 tall [R5]                              */
+                             0 = the library default, 8 x 8 tiles [R5]                                               */
   int32_t sort_mode;      /* LRA_SORT_TILE | LRA_SORT_TILE_CF [R5]                                             */
   double scale_u, scale_v; /* pixels per wavelength along u and v; sign allowed [R1]                            */
   int32_t n_cf;           /* number of kernels in the CF table                                                 */

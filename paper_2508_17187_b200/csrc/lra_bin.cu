@@ -1,7 +1,7 @@
 // lra_bin.cu -- coordinate/index kernel and the hand-written stable LSD radix sort behind lra_bin
 // ("re-ordering for runtime performance"; readings R2, R4, R5 in DESIGN.md).
 // Integer / fp64 work only; every output must be bit-exact against the oracle.
-#include "lra_internal.cuh"
+#include "lra_pipe.cuh"
 
 // ---------------------------------------------------------------------------------------------------
 // a1: coordinate / index.  One thread per visibility point k = r*nchan + c.
@@ -248,7 +248,7 @@ int lra_bin_impl(lra_plan* p, int64_t nrow, int32_t nchan, const double* uvw, co
   LRA_CUDA(p, cudaMemcpyAsync(p->d_su, su.data(), nchan * sizeof(double), cudaMemcpyHostToDevice, p->stream));
   LRA_CUDA(p, cudaMemcpyAsync(p->d_sv, sv.data(), nchan * sizeof(double), cudaMemcpyHostToDevice, p->stream));
   LRA_CUDA(p, cudaStreamSynchronize(p->stream));  // su / sv are stack-owned
-  LRA_CUDA(p, cudaMemsetAsync(p->counters, 0, 64 * sizeof(unsigned long long), p->stream));
+  LRA_CUDA(p, cudaMemsetAsync(p->counters, 0, LRA_TICKET0 * sizeof(unsigned long long), p->stream));
 
   unsigned long long per_tile = 1;
   if (p->sort_mode == LRA_SORT_TILE_CF) per_tile = (unsigned long long)p->n_cf * p->os * p->os;

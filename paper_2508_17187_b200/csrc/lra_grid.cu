@@ -4,7 +4,7 @@
 //   lra_sumwt_kernel        : sum of weights, per-thread fp64 partials -> block tree -> one atomic per block
 //   lra_grid_atomic_kernel  : variant 1, one CTA per visibility point, every tap a global float atomic (the
 //                             "before" design kept for profiling and as a second implementation in the tests)
-//   lra_grid_strip_kernel   : variant 0 (default), lra_grid_strip.cu
+//   lra_grid_region_kernel  : variant 0 (default), lra_grid_region.cu
 #include "lra_pipe.cuh"
 
 #define LRA_MAXG 16  // nterms * ncorr <= 4 * 4
@@ -68,7 +68,7 @@ lra_grid_atomic_kernel(const lra_rec* __restrict__ rec, const unsigned long long
   for (long long i = blockIdx.x; i < n; i += gridDim.x) {
     const lra_rec r = rec[i];
     const int ix = r.x & 0xffff, iy = r.x >> 16, S = r.w & 0xff, h = (S - 1) >> 1;
-    if (only_fallback && lra_group_of(S, tile_x, tile_y) != LRA_NGROUP - 1) continue;   // the strip kernels did those
+    if (only_fallback && lra_make_geom(S, tile_x, tile_y).group != LRA_NGROUP - 1) continue;   // the region kernels do those
     const float* slab = slabs + ((size_t)r.y << 2);
     const int pf = lra_plane_floats(S, tile_x);
     const uint32_t k = r.z;
@@ -105,8 +105,8 @@ lra_grid_atomic_kernel(const lra_rec* __restrict__ rec, const unsigned long long
   }
 }
 
-// defined in lra_grid_strip.cu
-int lra_grid_strip_launch(lra_plan* p, const float2* vis, const float* wt, const float* tau, float2* grid);
+// defined in lra_grid_region.cu
+int lra_grid_region_launch(lra_plan* p, const float2* vis, const float* wt, const float* tau, float2* grid);
 
 int lra_grid_impl(lra_plan* p, const float2* vis, const float* wt, const float* tau, float2* grid, double* sumwt) {
   if (p->npoints == 0) return LRA_OK;
@@ -116,12 +116,15 @@ int lra_grid_impl(lra_plan* p, const float2* vis, const float* wt, const float* 
     LRA_LAUNCH_CHECK(p);
   }
   const bool all_atomic = p->grid_variant == 1;
-  if (all_atomic || p->n_items[LRA_NGROUP - 1] > 0) {  // regions that fit no strip group (or the "before" variant)
+  bool fallback = false;
+  for (int c = 0; c < LRA_NCLASS; ++c)
+    if (p->n_items[c] > 0 && lra_make_geom(2 * c + 1, p->tile_x, p->tile).group == LRA_NGROUP - 1) fallback = true;
+  if (all_atomic || fallback) {  // regions that fit no group of the region kernel (or the "before" variant)
     lra_grid_atomic_kernel<<<p->sm_count * 16, 256, 0, p->stream>>>(p->rec, p->counters, p->slabs, vis, wt, tau,
                                                                      p->nchan, p->ncorr, p->nterms, p->nx, p->ny,
                                                                      p->tile_x, p->tile, all_atomic ? 0 : 1, grid);
     LRA_LAUNCH_CHECK(p);
     if (all_atomic) return LRA_OK;
   }
-  return lra_grid_strip_launch(p, vis, wt, tau, grid);
+  return lra_grid_region_launch(p, vis, wt, tau, grid);
 }

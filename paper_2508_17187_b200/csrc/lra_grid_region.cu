@@ -1,0 +1,349 @@
+// lra_grid_region.cu -- the default gridder (variant 0): region-owning CTAs that accumulate in REGISTERS with packed
+// fp32x2 FMAs and read the convolution function from a TMA-fed shared-memory ring.
+//
+// Operation: Eq. 7 / Eq. 23 of arxiv 2508.17187, tap loop of SURVEY Sec. 8(a) rows a3, a4.
+//
+// Design (B200-first; the paper's Kokkos kernel is prior art only):
+//   * lra_bin left the visibility points sorted by uv tile (8 x 8 pixels by default), then by CF slab.  A work item
+//     (lra_work.cu) is a run of at most LRA_CHUNK points of one tile and one support S; persistent CTAs take items
+//     through an atomic ticket, so the dense centre of a VLA-like uv plane is spread over many CTAs.
+//   * A CTA owns the item's region = tile + halo, RX x RY = (tile_x + S - 1) x (tile + S - 1) pixels, numbered
+//     linearly e = y*RX + x.  Consumer warp w owns, at step s, the 64 consecutive pixels from 64*(NW*s + w); a lane
+//     owns two of them, 32 apart.  The accumulators of those pixels stay in registers for the whole item and are
+//     added to the HBM grid once per item with red.global.add.v2.f32 (row a4).
+//   * The tile is small so that most of the region lies inside every footprint (S*S of (S+7)*(S+7) pixels): EVERY
+//     lane updates its pixels for EVERY point, with no test and no divergence.  The CF slab is stored with the
+//     region's pitch RX and zeros around the S x S taps (lra_internal.cuh), so the tap of pixel e for a point whose
+//     footprint starts at linear pixel `off` is simply slab[e - off]: a warp reads 32 CONSECUTIVE floats per load (no
+//     bank conflicts whatever RX is) and the lanes outside the footprint read zeros.
+//   * The tap update is done two pixels at a time with FFMA2 (fma.rn.f32x2): the pair (cre(e), cre(e+32))
+//     multiplies the point's duplicated value (vx, vx), so a complex multiply-add of two pixels on two grids is
+//     8 FFMA2 fed by 4 shared-memory loads -- the FP32 pipe and the shared-memory port saturate together.
+//   * lra_prepare_kernel first gathers vis / weight in SORTED order and writes wt*tau*V (in the duplicated form the
+//     FFMA2s want, with the point's slab offset beside it) as a contiguous stream.
+//   * The producer warp walks the batch stream of lra_work.cu and issues, per batch (= up to 12 slab runs of an
+//     item), TMA bulk copies (cp.async.bulk + mbarrier complete_tx): the prepared values of its points and its CF
+//     slabs, from L2 into a ring of shared-memory slots; item boundaries ride in the batch headers, so the consumers
+//     never touch the work list and synchronise once per batch, not once per slab.
+// Regions that fit no group (very large supports or tiles) take the global-atomic kernel of lra_grid.cu.
+#include <stdlib.h>
+
+#include "lra_pipe.cuh"
+
+struct lra_region_args {
+  const uint4* work;            // items of this launch's support class
+  unsigned n_items;
+  unsigned long long* ticket;
+  const uint4* batch;           // batch records of this class (4 x uint4 each)
+  const float* slabs;
+  const float* prep;            // this pass: [sorted position][NG][8]
+  float2* grid;                 // first grid of this pass
+  long long plane;              // pixels per grid
+  int nx, ny, tile_x, tile_y, ntx;
+  int S, rx, ry, ks;            // the class's geometry (lra_make_geom)
+  int core_bytes, stride_bytes, gap_bytes;   // slab plane as copied; plane + zeros; zeros before the first plane
+  int nslot, slot_bytes;        // ring geometry
+  int debug;                    // measurement aid (LRA_DEBUG env): 1 = consumers skip the taps, 2 = no slab copies
+};
+
+// slot layout (bytes): batch record (64) | pad | prepared values | slab area.  The slab area is gap, re plane of run
+// 0, gap, im plane of run 0, gap, re plane of run 1, ...: the kernel zeroes it once and the copies only ever write
+// the planes, so the gaps stay zero for the whole launch (one launch = one support class = one geometry).
+#define LRA_SLOT_VAL 128
+__host__ __device__ inline int lra_slot_slab0(int ng) { return LRA_SLOT_VAL + LRA_BATCH_POINTS * ng * 32; }
+#define LRA_RING_HDR 256   // full / empty barriers of up to 16 slots
+
+// wt * tau * V of every sorted point in the form the FFMA2s consume (reading R6: (wt*tau)*V in fp32):
+//   grid g = t*ncorr + p belongs to pass g/2; a pass holds [position][gl][8] = (vx, vx, vy, vy, -vy, -vy, pw, 0)
+// with pw (lra_pipe.cuh) in the record of the pass's first grid.
+__global__ void __launch_bounds__(256)
+lra_prepare_kernel(const lra_rec* __restrict__ rec, const unsigned long long* __restrict__ counters,
+                   const uint32_t* __restrict__ pw, const float2* __restrict__ vis, const float* __restrict__ wt,
+                   const float* __restrict__ tau, int nchan, int ncorr, int nterms, long long npoints,
+                   float4* __restrict__ prep) {
+  const long long n = (long long)counters[0] * ncorr;
+  const int ng = ncorr * nterms;
+  for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n; e += (long long)gridDim.x * blockDim.x) {
+    const long long i = e / ncorr;
+    const int p = (int)(e - i * ncorr);
+    const unsigned k = rec[i].z;
+    const float2 v = vis[(size_t)k * ncorr + p];
+    const float w = wt[(size_t)k * ncorr + p];
+    const float word = __uint_as_float(pw[i]);
+    const int c = (int)(k % (unsigned)nchan);
+    for (int t = 0; t < nterms; ++t) {
+      const float wgt = w * (tau ? tau[c * nterms + t] : 1.0f);
+      const float vx = wgt * v.x, vy = wgt * v.y;
+      const int g = t * ncorr + p, pass = g >> 1, gl = g & 1, ngp = ng - 2 * pass >= 2 ? 2 : 1;
+      float4* dst = prep + ((size_t)npoints * 2 * pass + (size_t)i * ngp + gl) * 2;
+      dst[0] = make_float4(vx, vx, vy, vy);
+      dst[1] = make_float4(-vy, -vy, word, 0.f);
+    }
+  }
+}
+
+// One step of one point: the two pixels (e, e + 32) this lane owns at step s, on NG grids.
+template <int NW, int NG>
+__device__ __forceinline__ void lra_grid_step(const float* __restrict__ re, const float* __restrict__ im, int s,
+                                              const lra_u64 (&vxx)[NG], const lra_u64 (&vyy)[NG],
+                                              const lra_u64 (&nvy)[NG], lra_u64 (&acc)[NG][2]) {
+  const lra_u64 cre = lra_pack2(re[s * 64 * NW], re[s * 64 * NW + 32]);
+  const lra_u64 cim = lra_pack2(im[s * 64 * NW], im[s * 64 * NW + 32]);
+#pragma unroll
+  for (int g = 0; g < NG; ++g) {
+    acc[g][0] = lra_fma2(cre, vxx[g], acc[g][0]);
+    acc[g][0] = lra_fma2(cim, nvy[g], acc[g][0]);
+    acc[g][1] = lra_fma2(cre, vyy[g], acc[g][1]);
+    acc[g][1] = lra_fma2(cim, vxx[g], acc[g][1]);
+  }
+}
+
+// Producer warp, shared by the gridder and the degridder: walks the items (atomic ticket) and their batches and
+// fills the ring: batch record, `val_bytes` per point from `vals` (if any) and the slab planes.
+template <int NW>
+__device__ __forceinline__ void lra_region_producer(const lra_region_args& a, const float* vals, uint32_t val_bytes,
+                                                    uint32_t slab0, uint32_t full0, uint32_t empty0, uint32_t slots0) {
+  const int lane = threadIdx.x & 31;
+  uint32_t slot = 0, par = 0;
+  for (;;) {
+    unsigned long long t = 0;
+    if (lane == 0) t = atomicAdd(a.ticket, 1ull);
+    t = __shfl_sync(0xffffffffu, t, 0);
+    if (t >= a.n_items) break;
+    const uint4 item = a.work[t];
+    const uint4* rec4 = a.batch + (size_t)item.y * 4;
+    uint4 nxt = make_uint4(0, 0, 0, 0);
+    if (lane < 4) nxt = rec4[lane];
+    for (unsigned b = 0; b < item.z; ++b) {
+      const uint4 cur = nxt;                              // lanes 0..3: the four quarters of batch b's record
+      if (b + 1 < item.z && lane < 4) nxt = rec4[(size_t)(b + 1) * 4 + lane];
+      const uint32_t sa = slots0 + slot * a.slot_bytes, fb = full0 + 8 * slot;
+      const uint32_t first = __shfl_sync(0xffffffffu, cur.x, 0);
+      const uint32_t count = __shfl_sync(0xffffffffu, cur.y, 0) & 0xff;
+      const uint32_t nr = __shfl_sync(0xffffffffu, cur.z, 0) & 0xff;
+      if (lane == 0) lra_mbar_wait(empty0 + 8 * slot, par ^ 1);
+      __syncwarp();
+      if (lane < 4)
+        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(sa + 16 * lane), "r"(cur.x), "r"(cur.y), "r"(cur.z), "r"(cur.w) : "memory");
+      __syncwarp();
+      const bool slabs = a.debug < 2;
+      if (lane == 0) {
+        lra_mbar_arrive_expect_tx(fb, (vals ? count * val_bytes : 0u) + (slabs ? nr * 2u * (uint32_t)a.core_bytes : 0u));
+        if (vals) lra_tma_load_1d(sa + LRA_SLOT_VAL, reinterpret_cast<const unsigned char*>(vals) + (size_t)first * val_bytes, count * val_bytes, fb);
+      }
+      // slab r of the batch: lane r / 4 + 1 holds its offset in component r % 4 of its quarter
+      for (uint32_t r = 0; r < nr; ++r) {
+        const uint32_t src = 1 + (r >> 2), c = r & 3;
+        const uint32_t pick = c == 0 ? cur.x : c == 1 ? cur.y : c == 2 ? cur.z : cur.w;
+        const uint32_t off16 = __shfl_sync(0xffffffffu, pick, src);
+        if (lane == 0 && slabs) {
+          const unsigned char* src_b = reinterpret_cast<const unsigned char*>(a.slabs) + ((size_t)off16 << 4);
+          const uint32_t dst = sa + slab0 + a.gap_bytes + r * 2 * a.stride_bytes;
+          lra_tma_load_1d(dst, src_b, a.core_bytes, fb);
+          lra_tma_load_1d(dst + a.stride_bytes, src_b + a.core_bytes, a.core_bytes, fb);
+        }
+      }
+      if (++slot == (uint32_t)a.nslot) { slot = 0; par ^= 1; }
+    }
+  }
+  if (lane == 0) {   // end marker
+    lra_mbar_wait(empty0 + 8 * slot, par ^ 1);
+    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(slots0 + slot * a.slot_bytes), "r"(0), "r"(LRA_BATCH_END), "r"(0), "r"(0) : "memory");
+    lra_mbar_arrive(full0 + 8 * slot);
+  }
+}
+
+// Ring set-up shared by the gridder and the degridder: barriers, zeroed slab areas.
+template <int NW>
+__device__ __forceinline__ void lra_region_ring_init(const lra_region_args& a, unsigned char* smem, int slab0,
+                                                     uint32_t full0, uint32_t empty0) {
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < a.nslot; ++s) { lra_mbar_init(full0 + 8 * s, 1); lra_mbar_init(empty0 + 8 * s, NW); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  const int area16 = (a.slot_bytes - slab0) >> 4;
+  for (int s = 0; s < a.nslot; ++s) {
+    uint4* z = reinterpret_cast<uint4*>(smem + LRA_RING_HDR + (size_t)s * a.slot_bytes + slab0);
+    for (int i = threadIdx.x; i < area16; i += (NW + 1) * 32) z[i] = make_uint4(0, 0, 0, 0);
+  }
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  __syncthreads();
+}
+
+template <int NW, int NG, int MINB>
+__global__ void __launch_bounds__((NW + 1) * 32, MINB) lra_grid_region_kernel(const lra_region_args a) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t sbase = lra_smem_u32(smem);
+  const uint32_t full0 = sbase, empty0 = sbase + 128, slots0 = sbase + LRA_RING_HDR;
+  const int slab0 = lra_slot_slab0(NG);
+  lra_region_ring_init<NW>(a, smem, slab0, full0, empty0);
+  if (warp == NW) {
+    lra_region_producer<NW>(a, a.prep, NG * 32, (uint32_t)slab0, full0, empty0, slots0);
+    return;
+  }
+  // -------------------------------------------------------------------- consumer warps
+  lra_u64 acc[LRA_KSMAX][NG][2];
+#pragma unroll
+  for (int s = 0; s < LRA_KSMAX; ++s)
+#pragma unroll
+    for (int g = 0; g < NG; ++g) acc[s][g][0] = acc[s][g][1] = 0ull;
+  uint32_t slot = 0, par = 0;
+  const int lane_off = slab0 + 4 * (64 * warp + lane);
+  const int ks = a.ks, im_off = a.stride_bytes;
+  for (;;) {
+    lra_mbar_wait(full0 + 8 * slot, par);
+    const unsigned char* sp = smem + LRA_RING_HDR + (size_t)slot * a.slot_bytes;
+    const uint4 h = *reinterpret_cast<const uint4*>(sp);
+    const unsigned count = a.debug >= 1 ? 0u : (h.y & 0xff);
+    const unsigned char* base = sp + lane_off;
+    const ulonglong2* vp = reinterpret_cast<const ulonglong2*>(sp + LRA_SLOT_VAL);
+    for (unsigned q = 0; q < count; ++q, vp += 2 * NG) {
+      lra_u64 vxx[NG], vyy[NG], nvy[NG];
+      const ulonglong2 v0 = vp[0], v1 = vp[1];
+      vxx[0] = v0.x; vyy[0] = v0.y; nvy[0] = v1.x;
+      if (NG == 2) {
+        const ulonglong2 v2 = vp[2];
+        vxx[NG - 1] = v2.x; vyy[NG - 1] = v2.y;
+        nvy[NG - 1] = reinterpret_cast<const lra_u64*>(vp)[6];
+      }
+      const float* re = reinterpret_cast<const float*>(base + (uint32_t)v1.y);
+      const float* im = reinterpret_cast<const float*>(base + (uint32_t)v1.y + im_off);
+      switch (ks) {   // steps are independent: enter at the class's step count and fall through
+        case 9: lra_grid_step<NW, NG>(re, im, 8, vxx, vyy, nvy, acc[8]);
+        case 8: lra_grid_step<NW, NG>(re, im, 7, vxx, vyy, nvy, acc[7]);
+        case 7: lra_grid_step<NW, NG>(re, im, 6, vxx, vyy, nvy, acc[6]);
+        case 6: lra_grid_step<NW, NG>(re, im, 5, vxx, vyy, nvy, acc[5]);
+        case 5: lra_grid_step<NW, NG>(re, im, 4, vxx, vyy, nvy, acc[4]);
+        case 4: lra_grid_step<NW, NG>(re, im, 3, vxx, vyy, nvy, acc[3]);
+        case 3: lra_grid_step<NW, NG>(re, im, 2, vxx, vyy, nvy, acc[2]);
+        case 2: lra_grid_step<NW, NG>(re, im, 1, vxx, vyy, nvy, acc[1]);
+        default: lra_grid_step<NW, NG>(re, im, 0, vxx, vyy, nvy, acc[0]);
+      }
+    }
+    __syncwarp();
+    if (lane == 0) lra_mbar_arrive(empty0 + 8 * slot);
+    if (h.y & LRA_BATCH_LAST) {
+      // ---- row a4: add the item's region to the grid, once ----
+      const int hh = (a.S - 1) >> 1;
+      const int ty = (int)(h.w / (unsigned)a.ntx), tx = (int)(h.w - (unsigned)ty * a.ntx);
+      const int x0 = tx * a.tile_x - hh, y0 = ty * a.tile_y - hh;
+      const unsigned magic = 0xffffffffu / (unsigned)a.rx + 1u;
+#pragma unroll
+      for (int s = 0; s < LRA_KSMAX; ++s) {
+        if (s < ks) {
+#pragma unroll
+          for (int half = 0; half < 2; ++half) {
+            const unsigned e = 64u * (NW * s + warp) + 32u * half + lane;
+            const int y = (int)__umulhi(e, magic), x = (int)e - y * a.rx;
+            const int gx = x0 + x, gy = y0 + y;
+            const bool ok = y < a.ry && gx >= 0 && gx < a.nx && gy >= 0 && gy < a.ny;
+#pragma unroll
+            for (int g = 0; g < NG; ++g) {
+              float r0, r1, i0, i1;
+              lra_unpack2(acc[s][g][0], r0, r1);
+              lra_unpack2(acc[s][g][1], i0, i1);
+              const float vr = half ? r1 : r0, vi = half ? i1 : i0;
+              if (ok && (vr != 0.f || vi != 0.f)) lra_red_add_v2(a.grid + (size_t)g * a.plane + (size_t)gy * a.nx + gx, vr, vi);
+            }
+          }
+#pragma unroll
+          for (int g = 0; g < NG; ++g) acc[s][g][0] = acc[s][g][1] = 0ull;
+        }
+      }
+    }
+    if (h.y & LRA_BATCH_END) break;
+    if (++slot == (uint32_t)a.nslot) { slot = 0; par ^= 1; }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Ring geometry of a class for a kernel whose slots start with `slab0` bytes of record + values.  Returns false if
+// not even one slot fits (the class then takes the fallback kernels).
+bool lra_region_ring(const lra_geom& q, int slab0, int ctas_per_sm, lra_region_args* a, int* smem_bytes) {
+  const int slab_area = 4 * (q.gap + q.per_batch * 2 * q.stride);
+  const int slot_bytes = (slab0 + slab_area + 127) & ~127;
+  const int budget = (227 * 1024) / ctas_per_sm - 1024 - LRA_RING_HDR;   // 1 KB per CTA is reserved by the system
+  int nslot = budget / slot_bytes;
+  if (nslot < 1) return false;
+  if (nslot > 6) nslot = 6;
+  const char* env = getenv("LRA_NSLOT");
+  if (env && atoi(env) >= 1 && atoi(env) < nslot) nslot = atoi(env);
+  a->S = q.S; a->rx = q.rx; a->ry = q.ry; a->ks = q.ks;
+  a->core_bytes = 4 * q.core; a->stride_bytes = 4 * q.stride; a->gap_bytes = 4 * q.gap;
+  a->nslot = nslot; a->slot_bytes = slot_bytes;
+  *smem_bytes = LRA_RING_HDR + nslot * slot_bytes;
+  return true;
+}
+
+template <int NW, int NG, int MINB>
+static int lra_launch_class(lra_plan* p, lra_region_args a, const lra_geom& q, int c, cudaStream_t st) {
+  int smem = 0;
+  if (!lra_region_ring(q, lra_slot_slab0(NG), MINB, &a, &smem)) return LRA_EINVAL;
+  auto kern = lra_grid_region_kernel<NW, NG, MINB>;
+  LRA_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  a.work = p->work + p->item_off[c];
+  a.n_items = (unsigned)p->n_items[c];
+  a.batch = reinterpret_cast<const uint4*>(p->batch) + (size_t)p->batch_off[c] * 4;
+  int ctas = p->sm_count * MINB;
+  if ((int64_t)ctas > p->n_items[c]) ctas = (int)p->n_items[c];
+  kern<<<ctas, (NW + 1) * 32, smem, st>>>(a);
+  LRA_LAUNCH_CHECK(p);
+  return LRA_OK;
+}
+
+int lra_grid_region_launch(lra_plan* p, const float2* vis, const float* wt, const float* tau, float2* grid) {
+  const int ng = p->ncorr * p->nterms;
+  const int64_t n = p->npoints;
+  int rc = LRA_OK;
+  // prepared values of all passes
+  const int64_t need = n * ng * 8;
+  if (need > p->prep_capacity) {
+    LRA_CUDA(p, cudaStreamSynchronize(p->stream));
+    if (p->prep) { cudaFree(p->prep); p->prep = nullptr; p->prep_capacity = 0; }
+    LRA_CUDA(p, cudaMalloc(&p->prep, (size_t)need * sizeof(float)));
+    p->prep_capacity = need;
+  }
+  lra_prepare_kernel<<<p->sm_count * 8, 256, 0, p->stream>>>(p->rec, p->counters, p->pw, vis, wt, tau, p->nchan, p->ncorr,
+                                                            p->nterms, (long long)n, (float4*)p->prep);
+  LRA_LAUNCH_CHECK(p);
+  LRA_CUDA(p, cudaMemsetAsync(p->counters + LRA_TICKET0, 0, LRA_NTICKET * sizeof(unsigned long long), p->stream));
+  lra_region_args a;
+  a.slabs = p->slabs;
+  a.plane = (long long)p->nx * p->ny;
+  a.nx = p->nx; a.ny = p->ny; a.tile_x = p->tile_x; a.tile_y = p->tile; a.ntx = p->ntx;
+  const char* dbg = getenv("LRA_DEBUG");
+  a.debug = dbg ? atoi(dbg) : 0;
+  // the per-class launches are independent: spread them over the plan's internal streams
+  LRA_CUDA(p, cudaEventRecord(p->ev_fork, p->stream));
+  for (int s = 0; s < LRA_NAUX; ++s) LRA_CUDA(p, cudaStreamWaitEvent(p->aux[s], p->ev_fork, 0));
+  int ticket = 0, turn = 0;
+  for (int pass = 0; 2 * pass < ng && rc == LRA_OK; ++pass) {
+    const int ngp = ng - 2 * pass >= 2 ? 2 : 1;
+    a.prep = p->prep + (size_t)n * 2 * pass * 8;
+    a.grid = grid + (size_t)(2 * pass) * a.plane;
+    for (int c = LRA_NCLASS - 1; c >= 0 && rc == LRA_OK; --c) {   // large supports first: their items are the longest
+      if (p->n_items[c] == 0) continue;
+      const lra_geom q = lra_make_geom(2 * c + 1, p->tile_x, p->tile);
+      if (q.group == LRA_NGROUP - 1) continue;                    // done by the fallback kernel
+      a.ticket = p->counters + LRA_TICKET0 + ticket++;
+      cudaStream_t st = p->aux[turn++ % LRA_NAUX];
+      if (ngp == 2) {
+        if (q.group == 0) rc = lra_launch_class<2, 2, 4>(p, a, q, c, st);
+        else if (q.group == 1) rc = lra_launch_class<4, 2, 3>(p, a, q, c, st);
+        else if (q.group == 2) rc = lra_launch_class<8, 2, 2>(p, a, q, c, st);
+        else rc = lra_launch_class<16, 2, 1>(p, a, q, c, st);
+      } else {
+        if (q.group == 0) rc = lra_launch_class<2, 1, 4>(p, a, q, c, st);
+        else if (q.group == 1) rc = lra_launch_class<4, 1, 3>(p, a, q, c, st);
+        else if (q.group == 2) rc = lra_launch_class<8, 1, 2>(p, a, q, c, st);
+        else rc = lra_launch_class<16, 1, 1>(p, a, q, c, st);
+      }
+    }
+  }
+  for (int s = 0; s < LRA_NAUX; ++s) {
+    LRA_CUDA(p, cudaEventRecord(p->ev_join[s], p->aux[s]));
+    LRA_CUDA(p, cudaStreamWaitEvent(p->stream, p->ev_join[s], 0));
+  }
+  return rc;
+}

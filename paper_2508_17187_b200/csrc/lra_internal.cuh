@@ -15,7 +15,9 @@
 //   w: S | cf << 8          (support in pixels, kernel number)
 typedef uint4 lra_rec;
 
-#define LRA_NGROUP 5   // kernel configurations of the strip gridder / degridder; the last one is the fallback
+#define LRA_NGROUP 5   // kernel configurations of the region gridder / degridder; the last one is the fallback
+#define LRA_NCLASS 65  // support classes: class (S - 1) / 2 for S = 1, 3, .., 129
+#define LRA_NAUX 4     // internal streams the per-class launches of one call are spread over
 
 struct lra_plan {
   // ---- descriptor (host copies) ----
@@ -51,17 +53,19 @@ struct lra_plan {
   unsigned long long* counters;  // see lra_pipe.cuh
   double *d_su, *d_sv;      // per-channel scale tables
   int32_t su_capacity;
-  // ---- work lists of the strip kernels (lra_work.cu; geometry only, rebuilt by every lra_bin) ----
-  uint4* work;              // items of all groups, grouped by group
+  // ---- work lists of the region kernels (lra_work.cu; geometry only, rebuilt by every lra_bin) ----
+  uint4* work;              // items of all classes, grouped by class
   int64_t work_capacity;
-  uint4* stage_hdr;         // stage headers of all groups, grouped by group; an item's stages are consecutive
-  int64_t stage_capacity;
-  uint32_t* pw;             // [npoints][16] per-point, per-consumer-warp words (tap offset | step mask << 16)
+  uint32_t* batch;          // batch records (16 words each), grouped by class; an item's are consecutive
+  int64_t batch_capacity;   // batches
+  uint32_t* pw;             // [npoints] per-point word (byte offset of the point's first tap in its batch's slab area)
   int64_t pw_capacity;      // points
   float* prep;              // gridder: wt*tau*V of every sorted point, FFMA2 operand form; degridder: sorted results
   int64_t prep_capacity;    // floats
-  int64_t n_items[8], item_off[8];     // items per group and first item of every group in `work`
-  int64_t n_stages[8], stage_off[8];   // stages per group and first stage of every group in `stage_hdr`
+  int64_t n_items[LRA_NCLASS], item_off[LRA_NCLASS];     // items per support class, first item of the class in `work`
+  int64_t n_batches[LRA_NCLASS], batch_off[LRA_NCLASS];  // batches per class, first batch of the class in `batch`
+  cudaStream_t aux[LRA_NAUX];          // per-class launches run concurrently on these, forked from / joined to `stream`
+  cudaEvent_t ev_fork, ev_join[LRA_NAUX];
   // ---- misc ----
   int32_t grid_variant, degrid_variant;
   int64_t launches;
@@ -70,14 +74,14 @@ struct lra_plan {
 };
 
 // Slab layout (one slab = the S*S taps of one kernel at one sub-pixel phase, what one visibility point needs).
-// A strip kernel works on a REGION of RX = S + tile_x - 1 columns (tile + halo) whose pixels are numbered
+// A region kernel works on a REGION of RX = S + tile_x - 1 columns (tile + halo) whose pixels are numbered
 // e = y*RX + x, and it reads the tap that a point with footprint origin (ox, oy) puts on pixel e at the linear
 // slab index e - (oy*RX + ox).  So a slab is stored with the region's pitch: two planes (real parts, then
-// imaginary parts) of PF = lra_plane_floats(S, tile_x) floats, tap (j, i), 0 <= j, i < S, at float j*RX + i, and
-// EVERY other float of the plane zero: the RX - S pad floats that end each row and the >= 64 floats that follow
-// the last row.  A lane that looks at a pixel outside the footprint therefore reads a zero instead of branching.
+// imaginary parts) of PF = lra_plane_floats(S, tile_x) floats, tap (j, i), 0 <= j, i < S, at float j*RX + i, and the
+// RX - S pad floats that end each row ZERO.  A lane that looks at a pixel beside the footprint therefore reads a
+// zero instead of branching (the zeros above and below the footprint live in shared memory, lra_pipe.cuh).
 // PF is a multiple of 4 (16 bytes) so that one TMA bulk copy moves a plane.
-__host__ __device__ inline int lra_plane_floats(int S, int tile_x) { return (S * (S + tile_x - 1) + 64 + 3) & ~3; }
+__host__ __device__ inline int lra_plane_floats(int S, int tile_x) { return (S * (S + tile_x - 1) + 3) & ~3; }
 __host__ __device__ inline int lra_tap_index(int S, int tile_x, int j, int i) { return j * (S + tile_x - 1) + i; }
 
 #define LRA_CUDA(p, call)                         \

@@ -6,48 +6,77 @@
 #include "lra_internal.cuh"
 
 #define LRA_CHUNK 1024     // sorted positions per work-list chunk = upper bound on the points of one work item
-#define LRA_RUNMAX 16      // points per pipeline stage
-#define LRA_PW_STRIDE 16   // per-point words: one per consumer warp, 16 = the largest warp count of a group
+#define LRA_RUNMAX 8       // points of one slab run inside a batch (longer runs are cut and load their slab again)
+#define LRA_BATCH_SLABS 12 // slab runs per batch at most
+#define LRA_BATCH_POINTS (LRA_RUNMAX * LRA_BATCH_SLABS)
+#define LRA_KSMAX 9        // steps per consumer warp at most: 9 * 2 pixels * 2 grids * (re, im) = 72 accumulators
 
 typedef unsigned long long lra_u64;
 
 // ---------------------------------------------------------------------------------------------------
-// Groups.  A strip kernel keeps a region of RX*RY pixels (tile + halo, RX = tile_x + S - 1, RY = tile + S - 1) in
-// the registers of NW consumer warps: pixel e = y*RX + x belongs to warp (e / 64) % NW, lane e % 32, step
-// e / (64*NW), half (e / 32) % 2, i.e. at step s a warp owns the 64 consecutive pixels that start at
-// 64*(NW*s + warp) and a lane owns two of them, 32 apart (the two halves of one FFMA2).  A group is one
-// compile-time choice of (NW, KS = steps); an item goes to the smallest group whose 64*NW*KS pixels hold its
-// region, and to the fallback group (global atomics, no limit) if none does.
+// Geometry of a support class.  A region kernel keeps a region of RX*RY pixels (tile + halo, RX = tile_x + S - 1,
+// RY = tile + S - 1) in the registers of NW consumer warps: pixel e = y*RX + x belongs to warp (e / 64) % NW, step
+// e / (64*NW), lane e % 32, half (e / 32) % 2, i.e. at step s a warp owns the 64 consecutive pixels that start at
+// 64*(NW*s + warp) and a lane owns two of them, 32 apart (the two halves of one FFMA2).  NW = 2, 4, 8 or 16 is the
+// smallest for which ks = ceil(RX*RY / (64*NW)) <= LRA_KSMAX; a region too large for NW = 16 goes to the fallback
+// kernels (global atomics).  Every lane reads a tap for every point, at linear slab index e - off with
+// off = oy*RX + ox <= pre, so a slab plane sits in shared memory between zeros: `gap` floats before (>= pre) and
+// after (>= the pixels past the last tap) -- consecutive planes share a gap, which no copy ever writes.
 // ---------------------------------------------------------------------------------------------------
-__host__ __device__ inline int lra_group_nw(int g) { return g == 0 ? 4 : g == 1 ? 8 : 16; }
-__host__ __device__ inline int lra_group_ks(int g) { return g == 0 ? 8 : g == 1 ? 8 : g == 2 ? 7 : 9; }
-__host__ __device__ inline int lra_group_slots(int g) { return 64 * lra_group_nw(g) * lra_group_ks(g); }
-__host__ __device__ inline int lra_group_of(int S, int tile_x, int tile_y) {
-  const int slots = (S + tile_x - 1) * (S + tile_y - 1);
+struct lra_geom {
+  int S, rx, ry, group, nw, ks;   // group = log2(nw) - 1, or LRA_NGROUP - 1 for the fallback
+  int core;                       // floats per slab plane as stored and copied (lra_plane_floats)
+  int gap, stride;                // floats of zeros between planes; stride = core + gap
+  int per_batch;                  // slab runs per batch
+};
+__host__ __device__ inline int lra_group_budget(int g) { return g == 0 ? 20480 : g == 1 ? 36864 : g == 2 ? 45056 : 81920; }
+__host__ __device__ inline lra_geom lra_make_geom(int S, int tile_x, int tile_y) {
+  lra_geom q;
+  q.S = S; q.rx = S + tile_x - 1; q.ry = S + tile_y - 1;
+  const int slots = q.rx * q.ry;
+  q.group = LRA_NGROUP - 1; q.nw = 0; q.ks = 0;
   for (int g = 0; g < LRA_NGROUP - 1; ++g)
-    if (slots <= lra_group_slots(g)) return g;
-  return LRA_NGROUP - 1;
+    if (slots <= 64 * (2 << g) * LRA_KSMAX) { q.group = g; q.nw = 2 << g; q.ks = (slots + 64 * q.nw - 1) / (64 * q.nw); break; }
+  q.core = lra_plane_floats(S, tile_x);
+  const int pre = (tile_y - 1) * q.rx + tile_x - 1, post = 64 * q.nw * q.ks - S * q.rx;
+  q.gap = ((pre > post ? pre : post) + 3) & ~3;
+  q.stride = q.core + q.gap;
+  q.per_batch = 1;
+  if (q.group < LRA_NGROUP - 1) {
+    const int r = lra_group_budget(q.group) / (8 * q.stride);
+    q.per_batch = r < 1 ? 1 : r > LRA_BATCH_SLABS ? LRA_BATCH_SLABS : r;
+  }
+  return q;
 }
+__host__ __device__ inline int lra_class_of(int S) { return (S - 1) >> 1; }
 
 // ---------------------------------------------------------------------------------------------------
-// Stage stream (built once per lra_bin by lra_work.cu; geometry only, reused by every lra_grid / lra_degrid).
+// Batch stream (built once per lra_bin by lra_work.cu; geometry only, reused by every lra_grid / lra_degrid).
 //   item  = maximal run of sorted positions with the same uv tile and the same support, cut at multiples of
-//           LRA_CHUNK: uint4 {tile id, first stage (group-relative), number of stages, S}.  One CTA accumulates an
-//           item's region in registers and adds it to the grid once.
-//   stage = run of at most LRA_RUNMAX points of one item that share one CF slab, i.e. what occupies one slot of a
-//           CTA's shared-memory ring: uint4 {first sorted position, count | S << 8 | flags, slab offset in
-//           16-byte units, tile id}.  LRA_STAGE_LAST marks the last stage of its item.
-//   pw    = for every sorted position, LRA_PW_STRIDE words, one per consumer warp w of the point's group:
-//           4*(oy*RX + ox) in the low half (byte offset of the point's footprint origin in the region) and, in
-//           the high half, bit s set <=> the 64 pixels warp w owns at step s meet the point's footprint.
+//           LRA_CHUNK: uint4 {tile id, first batch (class-relative), number of batches, S}.  One CTA accumulates an
+//           item's region in registers and adds it to the grid once.  Items are grouped by support class.
+//   run   = at most LRA_RUNMAX consecutive points of an item that share one CF slab.
+//   batch = per_batch consecutive runs of one item: what occupies one slot of a CTA's shared-memory ring.
+//           64 bytes: uint4 {first sorted position, count | flags, runs, tile id}, then the slab offsets of its
+//           runs in 16-byte units (uint32 x 12).  LRA_BATCH_LAST marks the last batch of its item.
+//   pw    = for every sorted position one word: the byte offset, inside the slot's slab area, of the float the
+//           lane that owns pixel 0 of the region reads for this point: 4 * (gap + run * 2 * stride - (oy*RX + ox)).
 // ---------------------------------------------------------------------------------------------------
-#define LRA_STAGE_LAST 0x40000000u
-#define LRA_STAGE_END 0x80000000u
+#define LRA_BATCH_LAST 0x40000000u
+#define LRA_BATCH_END 0x80000000u
 
-// counters[0] n_valid, [1] sum S^2, [8..15] items per group, [16..23] stages per group, [24..31] item cursors,
-// [32..39] stage cursors, [40..47] item offsets, [48..55] stage offsets, [64..127] work tickets of the launches.
-#define LRA_TICKET0 64
-#define LRA_NTICKET 64
+// counters (unsigned long long): [0] n_valid, [1] sum S^2; per support class c: [128 + c] items, [256 + c] batches,
+// [384 + c] item cursor, [512 + c] batch cursor, [640 + c] first item, [768 + c] first batch; [1024..2047] work
+// tickets of the launches of one call.
+#define LRA_NCOUNTER 2048
+#define LRA_CNT_ITEMS 128
+#define LRA_CNT_BATCHES 256
+#define LRA_CNT_ITEM_CUR 384
+#define LRA_CNT_BATCH_CUR 512
+#define LRA_CNT_ITEM_OFF 640
+#define LRA_CNT_BATCH_OFF 768
+#define LRA_TICKET0 1024
+#define LRA_NTICKET 1024
 
 // ---------------------------------------------------------------------------------------------------
 // PTX wrappers
@@ -94,30 +123,4 @@ __device__ __forceinline__ lra_u64 lra_pack2(float lo, float hi) {
 }
 __device__ __forceinline__ void lra_unpack2(lra_u64 v, float& lo, float& hi) {
   asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
-}
-__device__ __forceinline__ float lra_lds(uint32_t addr) {
-  float v;
-  asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
-  return v;
-}
-__device__ __forceinline__ uint32_t lra_lds_u32(uint32_t addr) {
-  uint32_t v;
-  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
-  return v;
-}
-__device__ __forceinline__ uint4 lra_lds_v4(uint32_t addr) {
-  uint4 v;
-  asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
-  return v;
-}
-__device__ __forceinline__ void lra_lds_2x64(uint32_t addr, lra_u64& a, lra_u64& b) {
-  asm volatile("ld.shared.v2.u64 {%0, %1}, [%2];" : "=l"(a), "=l"(b) : "r"(addr));
-}
-__device__ __forceinline__ lra_u64 lra_lds_u64(uint32_t addr) {
-  lra_u64 v;
-  asm volatile("ld.shared.u64 %0, [%1];" : "=l"(v) : "r"(addr));
-  return v;
-}
-__device__ __forceinline__ void lra_sts_v4(uint32_t addr, uint4 v) {
-  asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }

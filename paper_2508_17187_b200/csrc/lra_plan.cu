@@ -3,7 +3,7 @@
 #include <new>
 #include <string.h>
 
-#include "lra_internal.cuh"
+#include "lra_pipe.cuh"
 
 // Re-lay one oversampled kernel into phase-major planar slabs (reading R3; layout in
 // lra_internal.cuh):  tap (j + h, i + h) of slab (fyi, fxi) = K[(j*os - fy) + c0][(i*os - fx) + c0],
@@ -44,8 +44,8 @@ extern "C" int lra_plan_create(lra_plan** out, const lra_plan_desc* d) {
   if (!d || d->nx < 1 || d->ny < 1 || d->nx > 32768 || d->ny > 32768) return LRA_EINVAL;
   if (d->ncorr < 1 || d->ncorr > 4 || d->nterms < 1 || d->nterms > 4) return LRA_EINVAL;
   if (d->oversampling < 1 || d->oversampling > 64) return LRA_EINVAL;
-  // tile = 0: the library's default strip, 8 wide (u) by 64 tall (v); tile_x = 0 with tile != 0: square tiles
-  int tile = d->tile == 0 ? 64 : d->tile;
+  // tile = 0: the library's default, 8 x 8; tile_x = 0 with tile != 0: square tiles
+  int tile = d->tile == 0 ? 8 : d->tile;
   int tile_x = d->tile_x == 0 ? (d->tile == 0 ? 8 : tile) : d->tile_x;
   if (!is_pow2(tile) || tile < 4 || tile > 1024 || !is_pow2(tile_x) || tile_x < 4 || tile_x > 1024) return LRA_EINVAL;
   if (d->sort_mode != LRA_SORT_TILE && d->sort_mode != LRA_SORT_TILE_CF) return LRA_EINVAL;
@@ -89,8 +89,13 @@ extern "C" int lra_plan_create(lra_plan** out, const lra_plan_desc* d) {
   CK(cudaMalloc(&p->slabs, (size_t)total * sizeof(float)));
   CK(cudaMalloc(&p->d_cf_support, (size_t)d->n_cf * sizeof(int32_t)));
   CK(cudaMalloc(&p->d_slab_off, (size_t)d->n_cf * sizeof(int64_t)));
-  CK(cudaMalloc(&p->counters, 128 * sizeof(unsigned long long)));
-  CK(cudaMemsetAsync(p->counters, 0, 128 * sizeof(unsigned long long), p->stream));
+  CK(cudaMalloc(&p->counters, LRA_NCOUNTER * sizeof(unsigned long long)));
+  CK(cudaMemsetAsync(p->counters, 0, LRA_NCOUNTER * sizeof(unsigned long long), p->stream));
+  for (int s = 0; s < LRA_NAUX; ++s) {
+    CK(cudaStreamCreateWithFlags(&p->aux[s], cudaStreamNonBlocking));
+    CK(cudaEventCreateWithFlags(&p->ev_join[s], cudaEventDisableTiming));
+  }
+  CK(cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming));
   CK(cudaMalloc(&p->tile_start, (size_t)(p->ntiles + 1) * sizeof(uint32_t)));
   CK(cudaMemcpyAsync(p->d_cf_support, p->cf_support.data(), (size_t)d->n_cf * sizeof(int32_t), cudaMemcpyHostToDevice, p->stream));
   CK(cudaMemcpyAsync(p->d_slab_off, p->slab_off.data(), (size_t)d->n_cf * sizeof(int64_t), cudaMemcpyHostToDevice, p->stream));
@@ -122,9 +127,14 @@ extern "C" int lra_plan_destroy(lra_plan* p) {
   cudaSetDevice(p->device);
   cudaStreamSynchronize(p->stream);
   void* ptrs[] = {p->slabs, p->d_cf_support, p->d_slab_off, p->ix, p->iy, p->fx, p->fy, p->key, p->skey[0], p->skey[1],
-                  p->sval[0], p->sval[1], p->hist, p->tile_start, p->rec, p->counters, p->d_su, p->d_sv, p->work, p->stage_hdr, p->pw, p->prep};
+                  p->sval[0], p->sval[1], p->hist, p->tile_start, p->rec, p->counters, p->d_su, p->d_sv, p->work, p->batch, p->pw, p->prep};
   for (void* q : ptrs)
     if (q) cudaFree(q);
+  for (int s = 0; s < LRA_NAUX; ++s) {
+    if (p->aux[s]) { cudaStreamSynchronize(p->aux[s]); cudaStreamDestroy(p->aux[s]); }
+    if (p->ev_join[s]) cudaEventDestroy(p->ev_join[s]);
+  }
+  if (p->ev_fork) cudaEventDestroy(p->ev_fork);
   delete p;
   return LRA_OK;
 }

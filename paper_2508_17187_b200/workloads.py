@@ -64,7 +64,7 @@ class Config:
     time_stride_of: int = 0  # cfg5: take ntimes samples out of this many, 0 = off
     degrid: bool = False    # cfg5: model grid + degrid + residual gridding
     n_sources: int = 0
-    tile: int = 64          # uv tiles of the bucket sort: tile_x wide (u) by tile tall (v) -- the library's default strips
+    tile: int = 8           # uv tiles of the bucket sort: tile_x wide (u) by tile tall (v) -- the library's default
     tile_x: int = 8
 
     @property

@@ -10,7 +10,7 @@ pytestmark = pytest.mark.gpu
 
 torch = pytest.importorskip("torch")
 C_LIGHT = 299792458.0
-TILE = (8, 64)      # (tile_x, tile): the library's default strips, spelled out so that the oracle gets the same
+TILE = (8, 8)       # (tile_x, tile): the library's default tiles, spelled out so that the oracle gets the same
 
 
 @pytest.fixture(scope="module")
