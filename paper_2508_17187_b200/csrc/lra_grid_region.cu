@@ -42,7 +42,7 @@ struct lra_region_args {
   int nx, ny, tile_x, tile_y, ntx;
   int S, rx, ry, ks;            // the class's geometry (lra_make_geom)
   int core_bytes, stride_bytes, gap_bytes;   // slab plane as copied; plane + zeros; zeros before the first plane
-  int nslot, slot_bytes;        // ring geometry
+  int nslot, slot_bytes, slab0; // ring geometry: slots, bytes per slot, offset of the slab area inside a slot
   int debug;                    // measurement aid (LRA_DEBUG env): 1 = consumers skip the taps, 2 = no slab copies
 };
 
@@ -50,7 +50,6 @@ struct lra_region_args {
 // 0, gap, im plane of run 0, gap, re plane of run 1, ...: the kernel zeroes it once and the copies only ever write
 // the planes, so the gaps stay zero for the whole launch (one launch = one support class = one geometry).
 #define LRA_SLOT_VAL 128
-__host__ __device__ inline int lra_slot_slab0(int ng) { return LRA_SLOT_VAL + LRA_BATCH_POINTS * ng * 32; }
 #define LRA_RING_HDR 256   // full / empty barriers of up to 16 slots
 
 // wt * tau * V of every sorted point in the form the FFMA2s consume (reading R6: (wt*tau)*V in fp32):
@@ -102,48 +101,60 @@ __device__ __forceinline__ void lra_grid_step(const float* __restrict__ re, cons
 // fills the ring: batch record, `val_bytes` per point from `vals` (if any) and the slab planes.
 template <int NW>
 __device__ __forceinline__ void lra_region_producer(const lra_region_args& a, const float* vals, uint32_t val_bytes,
-                                                    uint32_t slab0, uint32_t full0, uint32_t empty0, uint32_t slots0) {
+                                                    uint32_t full0, uint32_t empty0, uint32_t slots0) {
   const int lane = threadIdx.x & 31;
+  const uint32_t slab0 = (uint32_t)a.slab0;
   uint32_t slot = 0, par = 0;
+  // tickets and item records are fetched one item ahead, batch records eight batches ahead: lane l of a group of
+  // eight batches holds quarter l % 4 of the record of batch l / 4
+  unsigned long long t_nxt = 0;
+  if (lane == 0) t_nxt = atomicAdd(a.ticket, 1ull);
+  t_nxt = __shfl_sync(0xffffffffu, t_nxt, 0);
+  uint4 item_nxt = make_uint4(0, 0, 0, 0);
+  if (t_nxt < a.n_items) item_nxt = a.work[t_nxt];
   for (;;) {
-    unsigned long long t = 0;
-    if (lane == 0) t = atomicAdd(a.ticket, 1ull);
-    t = __shfl_sync(0xffffffffu, t, 0);
-    if (t >= a.n_items) break;
-    const uint4 item = a.work[t];
+    if (t_nxt >= a.n_items) break;
+    const uint4 item = item_nxt;
+    if (lane == 0) t_nxt = atomicAdd(a.ticket, 1ull);
+    t_nxt = __shfl_sync(0xffffffffu, t_nxt, 0);
+    if (t_nxt < a.n_items) item_nxt = a.work[t_nxt];
     const uint4* rec4 = a.batch + (size_t)item.y * 4;
+    const unsigned nb = item.z;
     uint4 nxt = make_uint4(0, 0, 0, 0);
-    if (lane < 4) nxt = rec4[lane];
-    for (unsigned b = 0; b < item.z; ++b) {
-      const uint4 cur = nxt;                              // lanes 0..3: the four quarters of batch b's record
-      if (b + 1 < item.z && lane < 4) nxt = rec4[(size_t)(b + 1) * 4 + lane];
-      const uint32_t sa = slots0 + slot * a.slot_bytes, fb = full0 + 8 * slot;
-      const uint32_t first = __shfl_sync(0xffffffffu, cur.x, 0);
-      const uint32_t count = __shfl_sync(0xffffffffu, cur.y, 0) & 0xff;
-      const uint32_t nr = __shfl_sync(0xffffffffu, cur.z, 0) & 0xff;
-      if (lane == 0) lra_mbar_wait(empty0 + 8 * slot, par ^ 1);
-      __syncwarp();
-      if (lane < 4)
-        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(sa + 16 * lane), "r"(cur.x), "r"(cur.y), "r"(cur.z), "r"(cur.w) : "memory");
-      __syncwarp();
-      const bool slabs = a.debug < 2;
-      if (lane == 0) {
-        lra_mbar_arrive_expect_tx(fb, (vals ? count * val_bytes : 0u) + (slabs ? nr * 2u * (uint32_t)a.core_bytes : 0u));
-        if (vals) lra_tma_load_1d(sa + LRA_SLOT_VAL, reinterpret_cast<const unsigned char*>(vals) + (size_t)first * val_bytes, count * val_bytes, fb);
-      }
-      // slab r of the batch: lane r / 4 + 1 holds its offset in component r % 4 of its quarter
-      for (uint32_t r = 0; r < nr; ++r) {
-        const uint32_t src = 1 + (r >> 2), c = r & 3;
-        const uint32_t pick = c == 0 ? cur.x : c == 1 ? cur.y : c == 2 ? cur.z : cur.w;
-        const uint32_t off16 = __shfl_sync(0xffffffffu, pick, src);
-        if (lane == 0 && slabs) {
-          const unsigned char* src_b = reinterpret_cast<const unsigned char*>(a.slabs) + ((size_t)off16 << 4);
-          const uint32_t dst = sa + slab0 + a.gap_bytes + r * 2 * a.stride_bytes;
-          lra_tma_load_1d(dst, src_b, a.core_bytes, fb);
-          lra_tma_load_1d(dst + a.stride_bytes, src_b + a.core_bytes, a.core_bytes, fb);
+    if ((unsigned)(lane >> 2) < nb) nxt = rec4[lane];
+    for (unsigned b0 = 0; b0 < nb; b0 += 8) {
+      const uint4 cur = nxt;
+      if (b0 + 8 + (lane >> 2) < nb) nxt = rec4[(size_t)(b0 + 8) * 4 + lane];
+      const unsigned m = nb - b0 < 8u ? nb - b0 : 8u;
+      for (unsigned j = 0; j < m; ++j) {
+        // lane 4j owns the batch: slot hand-over, record, prepared values
+        const uint32_t sa = slots0 + slot * a.slot_bytes, fb = full0 + 8 * slot;
+        const uint32_t nr = __shfl_sync(0xffffffffu, cur.z, 4 * j) & 0xff;
+        const bool slabs = a.debug < 2;
+        if (lane == (int)(4 * j)) {
+          const uint32_t count = cur.y & 0xff;
+          const bool pv = vals && a.debug < 3;
+          lra_mbar_wait(empty0 + 8 * slot, par ^ 1);
+          asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(sa), "r"(cur.x), "r"(cur.y), "r"(cur.z), "r"(cur.w) : "memory");
+          lra_mbar_arrive_expect_tx(fb, (pv ? count * val_bytes : 0u) + (slabs ? nr * 2u * (uint32_t)a.core_bytes : 0u));
+          if (pv) lra_tma_load_1d(sa + LRA_SLOT_VAL, reinterpret_cast<const unsigned char*>(vals) + (size_t)cur.x * val_bytes, count * val_bytes, fb);
         }
+        __syncwarp();   // the slot is free from here on
+        // one lane issues every slab copy (copies issued from several lanes were measured 20 % slower); slab r of the
+        // batch: quarter r / 4 + 1 of its record holds the offset in component r % 4
+        for (uint32_t r = 0; r < nr; ++r) {
+          const uint32_t c = r & 3;
+          const uint32_t pick = c == 0 ? cur.x : c == 1 ? cur.y : c == 2 ? cur.z : cur.w;
+          const uint32_t off16 = __shfl_sync(0xffffffffu, pick, 4 * j + 1 + (r >> 2));
+          if (lane == 0 && slabs) {
+            const unsigned char* src_b = reinterpret_cast<const unsigned char*>(a.slabs) + ((size_t)off16 << 4);
+            const uint32_t dst = sa + slab0 + a.gap_bytes + r * 2 * a.stride_bytes;
+            lra_tma_load_1d(dst, src_b, a.core_bytes, fb);
+            lra_tma_load_1d(dst + a.stride_bytes, src_b + a.core_bytes, a.core_bytes, fb);
+          }
+        }
+        if (++slot == (uint32_t)a.nslot) { slot = 0; par ^= 1; }
       }
-      if (++slot == (uint32_t)a.nslot) { slot = 0; par ^= 1; }
     }
   }
   if (lane == 0) {   // end marker
@@ -155,8 +166,9 @@ __device__ __forceinline__ void lra_region_producer(const lra_region_args& a, co
 
 // Ring set-up shared by the gridder and the degridder: barriers, zeroed slab areas.
 template <int NW>
-__device__ __forceinline__ void lra_region_ring_init(const lra_region_args& a, unsigned char* smem, int slab0,
+__device__ __forceinline__ void lra_region_ring_init(const lra_region_args& a, unsigned char* smem,
                                                      uint32_t full0, uint32_t empty0) {
+  const int slab0 = a.slab0;
   if (threadIdx.x == 0) {
     for (int s = 0; s < a.nslot; ++s) { lra_mbar_init(full0 + 8 * s, 1); lra_mbar_init(empty0 + 8 * s, NW); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -170,27 +182,26 @@ __device__ __forceinline__ void lra_region_ring_init(const lra_region_args& a, u
   __syncthreads();
 }
 
-template <int NW, int NG, int MINB>
-__global__ void __launch_bounds__((NW + 1) * 32, MINB) lra_grid_region_kernel(const lra_region_args a) {
+template <int NW, int KS, int NG>
+__global__ void __launch_bounds__((NW + 1) * 32, lra_ctas_per_sm(NW, KS)) lra_grid_region_kernel(const lra_region_args a) {
   extern __shared__ __align__(128) unsigned char smem[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t sbase = lra_smem_u32(smem);
   const uint32_t full0 = sbase, empty0 = sbase + 128, slots0 = sbase + LRA_RING_HDR;
-  const int slab0 = lra_slot_slab0(NG);
-  lra_region_ring_init<NW>(a, smem, slab0, full0, empty0);
+  lra_region_ring_init<NW>(a, smem, full0, empty0);
   if (warp == NW) {
-    lra_region_producer<NW>(a, a.prep, NG * 32, (uint32_t)slab0, full0, empty0, slots0);
+    lra_region_producer<NW>(a, a.prep, NG * 32, full0, empty0, slots0);
     return;
   }
   // -------------------------------------------------------------------- consumer warps
-  lra_u64 acc[LRA_KSMAX][NG][2];
+  lra_u64 acc[KS][NG][2];
 #pragma unroll
-  for (int s = 0; s < LRA_KSMAX; ++s)
+  for (int s = 0; s < KS; ++s)
 #pragma unroll
     for (int g = 0; g < NG; ++g) acc[s][g][0] = acc[s][g][1] = 0ull;
   uint32_t slot = 0, par = 0;
-  const int lane_off = slab0 + 4 * (64 * warp + lane);
-  const int ks = a.ks, im_off = a.stride_bytes;
+  const int lane_off = a.slab0 + 4 * (64 * warp + lane);
+  const int im_off = a.stride_bytes;
   for (;;) {
     lra_mbar_wait(full0 + 8 * slot, par);
     const unsigned char* sp = smem + LRA_RING_HDR + (size_t)slot * a.slot_bytes;
@@ -209,29 +220,20 @@ __global__ void __launch_bounds__((NW + 1) * 32, MINB) lra_grid_region_kernel(co
       }
       const float* re = reinterpret_cast<const float*>(base + (uint32_t)v1.y);
       const float* im = reinterpret_cast<const float*>(base + (uint32_t)v1.y + im_off);
-      switch (ks) {   // steps are independent: enter at the class's step count and fall through
-        case 9: lra_grid_step<NW, NG>(re, im, 8, vxx, vyy, nvy, acc[8]);
-        case 8: lra_grid_step<NW, NG>(re, im, 7, vxx, vyy, nvy, acc[7]);
-        case 7: lra_grid_step<NW, NG>(re, im, 6, vxx, vyy, nvy, acc[6]);
-        case 6: lra_grid_step<NW, NG>(re, im, 5, vxx, vyy, nvy, acc[5]);
-        case 5: lra_grid_step<NW, NG>(re, im, 4, vxx, vyy, nvy, acc[4]);
-        case 4: lra_grid_step<NW, NG>(re, im, 3, vxx, vyy, nvy, acc[3]);
-        case 3: lra_grid_step<NW, NG>(re, im, 2, vxx, vyy, nvy, acc[2]);
-        case 2: lra_grid_step<NW, NG>(re, im, 1, vxx, vyy, nvy, acc[1]);
-        default: lra_grid_step<NW, NG>(re, im, 0, vxx, vyy, nvy, acc[0]);
-      }
+#pragma unroll
+      for (int s = 0; s < KS; ++s) lra_grid_step<NW, NG>(re, im, s, vxx, vyy, nvy, acc[s]);
     }
     __syncwarp();
     if (lane == 0) lra_mbar_arrive(empty0 + 8 * slot);
-    if (h.y & LRA_BATCH_LAST) {
+    if ((h.y & LRA_BATCH_LAST) && a.debug < 4) {
       // ---- row a4: add the item's region to the grid, once ----
       const int hh = (a.S - 1) >> 1;
       const int ty = (int)(h.w / (unsigned)a.ntx), tx = (int)(h.w - (unsigned)ty * a.ntx);
       const int x0 = tx * a.tile_x - hh, y0 = ty * a.tile_y - hh;
       const unsigned magic = 0xffffffffu / (unsigned)a.rx + 1u;
 #pragma unroll
-      for (int s = 0; s < LRA_KSMAX; ++s) {
-        if (s < ks) {
+      for (int s = 0; s < KS; ++s) {
+        {
 #pragma unroll
           for (int half = 0; half < 2; ++half) {
             const unsigned e = 64u * (NW * s + warp) + 32u * half + lane;
@@ -258,38 +260,70 @@ __global__ void __launch_bounds__((NW + 1) * 32, MINB) lra_grid_region_kernel(co
 }
 
 // ---------------------------------------------------------------------------------------------------
-// Ring geometry of a class for a kernel whose slots start with `slab0` bytes of record + values.  Returns false if
-// not even one slot fits (the class then takes the fallback kernels).
-bool lra_region_ring(const lra_geom& q, int slab0, int ctas_per_sm, lra_region_args* a, int* smem_bytes) {
-  const int slab_area = 4 * (q.gap + q.per_batch * 2 * q.stride);
-  const int slot_bytes = (slab0 + slab_area + 127) & ~127;
-  const int budget = (227 * 1024) / ctas_per_sm - 1024 - LRA_RING_HDR;   // 1 KB per CTA is reserved by the system
-  int nslot = budget / slot_bytes;
+// Ring geometry of a class for a kernel that keeps `val_bytes` per point in the slot.  Returns false if not even
+// one slot fits (the class then takes the fallback kernels).
+bool lra_region_ring(const lra_geom& q, int val_bytes, lra_region_args* a, int* smem_bytes) {
+  const int slab0 = (LRA_SLOT_VAL + q.per_batch * LRA_RUNMAX * val_bytes + 127) & ~127;
+  const int slot_bytes = (slab0 + 4 * (q.gap + q.per_batch * 2 * q.stride) + 127) & ~127;
+  int nslot = (lra_cta_smem(q.nw, q.ks) - LRA_RING_HDR) / slot_bytes;
   if (nslot < 1) return false;
-  if (nslot > 6) nslot = 6;
+  if (nslot > 4) nslot = 4;
   const char* env = getenv("LRA_NSLOT");
   if (env && atoi(env) >= 1 && atoi(env) < nslot) nslot = atoi(env);
   a->S = q.S; a->rx = q.rx; a->ry = q.ry; a->ks = q.ks;
   a->core_bytes = 4 * q.core; a->stride_bytes = 4 * q.stride; a->gap_bytes = 4 * q.gap;
-  a->nslot = nslot; a->slot_bytes = slot_bytes;
+  a->nslot = nslot; a->slot_bytes = slot_bytes; a->slab0 = slab0;
   *smem_bytes = LRA_RING_HDR + nslot * slot_bytes;
   return true;
 }
 
-template <int NW, int NG, int MINB>
+template <int NW, int KS, int NG>
 static int lra_launch_class(lra_plan* p, lra_region_args a, const lra_geom& q, int c, cudaStream_t st) {
   int smem = 0;
-  if (!lra_region_ring(q, lra_slot_slab0(NG), MINB, &a, &smem)) return LRA_EINVAL;
-  auto kern = lra_grid_region_kernel<NW, NG, MINB>;
+  if (!lra_region_ring(q, NG * 32, &a, &smem)) return LRA_EINVAL;
+  auto kern = lra_grid_region_kernel<NW, KS, NG>;
   LRA_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
   a.work = p->work + p->item_off[c];
   a.n_items = (unsigned)p->n_items[c];
   a.batch = reinterpret_cast<const uint4*>(p->batch) + (size_t)p->batch_off[c] * 4;
-  int ctas = p->sm_count * MINB;
+  int ctas = p->sm_count * lra_ctas_per_sm(NW, KS);
   if ((int64_t)ctas > p->n_items[c]) ctas = (int)p->n_items[c];
   kern<<<ctas, (NW + 1) * 32, smem, st>>>(a);
   LRA_LAUNCH_CHECK(p);
   return LRA_OK;
+}
+
+template <int NW, int NG>
+static int lra_launch_class_ks(lra_plan* p, const lra_region_args& a, const lra_geom& q, int c, cudaStream_t st) {
+  switch (q.ks) {
+    case 1: return lra_launch_class<NW, 1, NG>(p, a, q, c, st);
+    case 2: return lra_launch_class<NW, 2, NG>(p, a, q, c, st);
+    case 3: return lra_launch_class<NW, 3, NG>(p, a, q, c, st);
+    case 4: return lra_launch_class<NW, 4, NG>(p, a, q, c, st);
+    case 5: return lra_launch_class<NW, 5, NG>(p, a, q, c, st);
+    case 6: return lra_launch_class<NW, 6, NG>(p, a, q, c, st);
+    default: break;
+  }
+  if constexpr (lra_ks_max(NW) > 6) {
+    switch (q.ks) {
+      case 7: return lra_launch_class<NW, 7, NG>(p, a, q, c, st);
+      case 8: return lra_launch_class<NW, 8, NG>(p, a, q, c, st);
+      case 9: return lra_launch_class<NW, 9, NG>(p, a, q, c, st);
+      default: break;
+    }
+  }
+  return LRA_EINVAL;
+}
+
+template <int NG>
+static int lra_launch_class_nw(lra_plan* p, const lra_region_args& a, const lra_geom& q, int c, cudaStream_t st) {
+  switch (q.nw) {
+    case 2: return lra_launch_class_ks<2, NG>(p, a, q, c, st);
+    case 4: return lra_launch_class_ks<4, NG>(p, a, q, c, st);
+    case 8: return lra_launch_class_ks<8, NG>(p, a, q, c, st);
+    case 16: return lra_launch_class_ks<16, NG>(p, a, q, c, st);
+    default: return LRA_EINVAL;
+  }
 }
 
 int lra_grid_region_launch(lra_plan* p, const float2* vis, const float* wt, const float* tau, float2* grid) {
@@ -328,17 +362,7 @@ int lra_grid_region_launch(lra_plan* p, const float2* vis, const float* wt, cons
       if (q.group == LRA_NGROUP - 1) continue;                    // done by the fallback kernel
       a.ticket = p->counters + LRA_TICKET0 + ticket++;
       cudaStream_t st = p->aux[turn++ % LRA_NAUX];
-      if (ngp == 2) {
-        if (q.group == 0) rc = lra_launch_class<2, 2, 4>(p, a, q, c, st);
-        else if (q.group == 1) rc = lra_launch_class<4, 2, 3>(p, a, q, c, st);
-        else if (q.group == 2) rc = lra_launch_class<8, 2, 2>(p, a, q, c, st);
-        else rc = lra_launch_class<16, 2, 1>(p, a, q, c, st);
-      } else {
-        if (q.group == 0) rc = lra_launch_class<2, 1, 4>(p, a, q, c, st);
-        else if (q.group == 1) rc = lra_launch_class<4, 1, 3>(p, a, q, c, st);
-        else if (q.group == 2) rc = lra_launch_class<8, 1, 2>(p, a, q, c, st);
-        else rc = lra_launch_class<16, 1, 1>(p, a, q, c, st);
-      }
+      rc = ngp == 2 ? lra_launch_class_nw<2>(p, a, q, c, st) : lra_launch_class_nw<1>(p, a, q, c, st);
     }
   }
   for (int s = 0; s < LRA_NAUX; ++s) {

@@ -6,7 +6,7 @@
 #include "lra_internal.cuh"
 
 #define LRA_CHUNK 1024     // sorted positions per work-list chunk = upper bound on the points of one work item
-#define LRA_RUNMAX 8       // points of one slab run inside a batch (longer runs are cut and load their slab again)
+#define LRA_RUNMAX 4       // points of one slab run inside a batch (longer runs are cut and load their slab again)
 #define LRA_BATCH_SLABS 12 // slab runs per batch at most
 #define LRA_BATCH_POINTS (LRA_RUNMAX * LRA_BATCH_SLABS)
 #define LRA_KSMAX 9        // steps per consumer warp at most: 9 * 2 pixels * 2 grids * (re, im) = 72 accumulators
@@ -18,8 +18,8 @@ typedef unsigned long long lra_u64;
 // RY = tile + S - 1) in the registers of NW consumer warps: pixel e = y*RX + x belongs to warp (e / 64) % NW, step
 // e / (64*NW), lane e % 32, half (e / 32) % 2, i.e. at step s a warp owns the 64 consecutive pixels that start at
 // 64*(NW*s + warp) and a lane owns two of them, 32 apart (the two halves of one FFMA2).  NW = 2, 4, 8 or 16 is the
-// smallest for which ks = ceil(RX*RY / (64*NW)) <= LRA_KSMAX; a region too large for NW = 16 goes to the fallback
-// kernels (global atomics).  Every lane reads a tap for every point, at linear slab index e - off with
+// smallest for which ks = ceil(RX*RY / (64*NW)) <= lra_ks_max(NW) (the register budget that still leaves two CTAs of
+// NW = 8 on an SM); a region too large for NW = 16 goes to the fallback kernels (global atomics).  Every lane reads a tap for every point, at linear slab index e - off with
 // off = oy*RX + ox <= pre, so a slab plane sits in shared memory between zeros: `gap` floats before (>= pre) and
 // after (>= the pixels past the last tap) -- consecutive planes share a gap, which no copy ever writes.
 // ---------------------------------------------------------------------------------------------------
@@ -29,21 +29,28 @@ struct lra_geom {
   int gap, stride;                // floats of zeros between planes; stride = core + gap
   int per_batch;                  // slab runs per batch
 };
-__host__ __device__ inline int lra_group_budget(int g) { return g == 0 ? 20480 : g == 1 ? 36864 : g == 2 ? 45056 : 81920; }
+__host__ __device__ constexpr int lra_ks_max(int nw) { return nw == 8 ? 6 : LRA_KSMAX; }
+// CTAs per SM the (NW, KS) kernel is built for: ~12 registers per step (8 accumulators, 4 taps in flight) + 36.
+__host__ __device__ constexpr int lra_ctas_per_sm(int nw, int ks) {
+  const int regs = (12 * ks + 36 + 7) / 8 * 8, r = 65536 / ((nw + 1) * 32 * regs);
+  return r < 1 ? 1 : r > 6 ? 6 : r;
+}
+// Shared memory of a CTA and of one ring slot (3 slots per CTA at least, whenever a slab fits).
+__host__ __device__ constexpr int lra_cta_smem(int nw, int ks) { return (227 * 1024) / lra_ctas_per_sm(nw, ks) - 1024; }
 __host__ __device__ inline lra_geom lra_make_geom(int S, int tile_x, int tile_y) {
   lra_geom q;
   q.S = S; q.rx = S + tile_x - 1; q.ry = S + tile_y - 1;
   const int slots = q.rx * q.ry;
   q.group = LRA_NGROUP - 1; q.nw = 0; q.ks = 0;
   for (int g = 0; g < LRA_NGROUP - 1; ++g)
-    if (slots <= 64 * (2 << g) * LRA_KSMAX) { q.group = g; q.nw = 2 << g; q.ks = (slots + 64 * q.nw - 1) / (64 * q.nw); break; }
+    if (slots <= 64 * (2 << g) * lra_ks_max(2 << g)) { q.group = g; q.nw = 2 << g; q.ks = (slots + 64 * q.nw - 1) / (64 * q.nw); break; }
   q.core = lra_plane_floats(S, tile_x);
   const int pre = (tile_y - 1) * q.rx + tile_x - 1, post = 64 * q.nw * q.ks - S * q.rx;
   q.gap = ((pre > post ? pre : post) + 3) & ~3;
   q.stride = q.core + q.gap;
   q.per_batch = 1;
-  if (q.group < LRA_NGROUP - 1) {
-    const int r = lra_group_budget(q.group) / (8 * q.stride);
+  if (q.group < LRA_NGROUP - 1) {   // a third of the CTA's shared memory per slot: 384 bytes of values + a slab per run
+    const int r = ((lra_cta_smem(q.nw, q.ks) - 512) / 3 - 256 - 4 * q.gap) / (LRA_RUNMAX * 64 + 8 * q.stride);
     q.per_batch = r < 1 ? 1 : r > LRA_BATCH_SLABS ? LRA_BATCH_SLABS : r;
   }
   return q;
