@@ -4,11 +4,13 @@
 // fp32 multiply-add; per-lane partial sums over taps, then a warp-shuffle tree.
 //
 // Kernels:
-//   lra_degrid_init_kernel : vis_out = vis_in (or 0) for every sample, so that points dropped by lra_bin get V = 0
-//   lra_degrid_warp_kernel : one warp per sorted visibility point.  Points are visited in tile order, so the
+//   lra_degrid_init_kernel   : vis_out = vis_in (or 0) for every sample, so that points dropped by lra_bin get V = 0
+//   lra_degrid_region_kernel : variant 0 (default), lra_degrid_region.cu
+//   lra_degrid_warp_kernel   : variant 1 and the fallback for regions too large for the region kernel: one warp per
+//                            sorted visibility point.  Points are visited in tile order, so the
 //                            warps resident on an SM read overlapping grid patches (L1 / L2 hits) and, with
 //                            LRA_SORT_TILE_CF, the same CF slabs.
-#include "lra_internal.cuh"
+#include "lra_pipe.cuh"
 
 __global__ void __launch_bounds__(256)
 lra_degrid_init_kernel(const float2* __restrict__ vis_in, float2* __restrict__ vis_out, long long nsamples) {
@@ -20,7 +22,8 @@ template <int NC>
 __global__ void __launch_bounds__(256)
 lra_degrid_warp_kernel(const lra_rec* __restrict__ rec, const unsigned long long* __restrict__ counters,
                        const float* __restrict__ slabs, const float2* __restrict__ grid, const float* __restrict__ tau,
-                       const float2* vis_in, float2* vis_out, int nchan, int nterms, int nx, int ny, int tile_x) {
+                       const float2* vis_in, float2* vis_out, int nchan, int nterms, int nx, int ny, int tile_x, int tile_y,
+                       int only_fallback) {
   const long long n = (long long)counters[0];
   const size_t plane = (size_t)nx * ny;
   const int lane = threadIdx.x & 31;
@@ -29,6 +32,7 @@ lra_degrid_warp_kernel(const lra_rec* __restrict__ rec, const unsigned long long
   for (long long i = warp0; i < n; i += nwarps) {
     const lra_rec r = rec[i];
     const int ix = r.x & 0xffff, iy = r.x >> 16, S = r.w & 0xff, h = (S - 1) >> 1;
+    if (only_fallback && lra_make_geom(S, tile_x, tile_y).group != LRA_NGROUP - 1) continue;   // the region kernels do those
     const float* slab = slabs + ((size_t)r.y << 2);
     const int pf = lra_plane_floats(S, tile_x);
     const unsigned k = r.z;
@@ -82,6 +86,9 @@ lra_degrid_warp_kernel(const lra_rec* __restrict__ rec, const unsigned long long
   }
 }
 
+// defined in lra_degrid_region.cu
+int lra_degrid_region_launch(lra_plan* p, const float2* grid, const float* tau, const float2* vis_in, float2* vis_out);
+
 int lra_degrid_impl(lra_plan* p, const float2* grid, const float* tau, const float2* vis_in, float2* vis_out) {
   if (p->npoints == 0) return LRA_OK;
   const long long nsamples = p->npoints * (long long)p->ncorr;
@@ -89,17 +96,25 @@ int lra_degrid_impl(lra_plan* p, const float2* grid, const float* tau, const flo
     lra_degrid_init_kernel<<<p->sm_count * 8, 256, 0, p->stream>>>(vis_in, vis_out, nsamples);
     LRA_LAUNCH_CHECK(p);
   }
-  const int blocks = p->sm_count * 8;
+  const bool all_warp = p->degrid_variant == 1;
+  bool fallback = false;
+  for (int c = 0; c < LRA_NCLASS; ++c)
+    if (p->n_items[c] > 0 && lra_make_geom(2 * c + 1, p->tile_x, p->tile).group == LRA_NGROUP - 1) fallback = true;
+  if (all_warp || fallback) {   // regions that fit no group of the region kernel (or the "before" variant)
+    const int blocks = p->sm_count * 8;
 #define LRA_DG(NC)                                                                                                  \
   lra_degrid_warp_kernel<NC><<<blocks, 256, 0, p->stream>>>(p->rec, p->counters, p->slabs, grid, tau, vis_in, vis_out, \
-                                                            p->nchan, p->nterms, p->nx, p->ny, p->tile_x)
-  switch (p->ncorr) {
-    case 1: LRA_DG(1); break;
-    case 2: LRA_DG(2); break;
-    case 3: LRA_DG(3); break;
-    default: LRA_DG(4); break;
-  }
+                                                            p->nchan, p->nterms, p->nx, p->ny, p->tile_x, p->tile,    \
+                                                            all_warp ? 0 : 1)
+    switch (p->ncorr) {
+      case 1: LRA_DG(1); break;
+      case 2: LRA_DG(2); break;
+      case 3: LRA_DG(3); break;
+      default: LRA_DG(4); break;
+    }
 #undef LRA_DG
-  LRA_LAUNCH_CHECK(p);
-  return LRA_OK;
+    LRA_LAUNCH_CHECK(p);
+    if (all_warp) return LRA_OK;
+  }
+  return lra_degrid_region_launch(p, grid, tau, vis_in, vis_out);
 }

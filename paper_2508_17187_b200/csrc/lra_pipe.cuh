@@ -66,7 +66,7 @@ __host__ __device__ inline int lra_class_of(int S) { return (S - 1) >> 1; }
 //   batch = per_batch consecutive runs of one item: what occupies one slot of a CTA's shared-memory ring.
 //           64 bytes: uint4 {first sorted position, count | flags, runs, tile id}, then the slab offsets of its
 //           runs in 16-byte units (uint32 x 12).  LRA_BATCH_LAST marks the last batch of its item.
-//   pw    = for every sorted position one word: the byte offset, inside the slot's slab area, of the float the
+//   pw    = for every sorted position 16 bytes (one TMA granule), first word: the byte offset, inside the slot's slab area, of the float the
 //           lane that owns pixel 0 of the region reads for this point: 4 * (gap + run * 2 * stride - (oy*RX + ox)).
 // ---------------------------------------------------------------------------------------------------
 #define LRA_BATCH_LAST 0x40000000u
