@@ -2,7 +2,7 @@
 """bench.py -- one JSON line for the gridding / degridding hot path on B200.
 
 A "step" is one pass of the whole hot path over one batch of synthetic input:
-lra_bin (index + bucket sort) -> lra_grid (tap loop + tile flush + sum of weights) -> lra_degrid (model
+lra_bin (index + bucket sort) -> lra_grid (tap loop + region flush + sum of weights) -> lra_degrid (model
 prediction with the fused residual).  Workload at N = 1: BASELINE.json configs[2], the VLA-like W-projection
 configuration the target is quoted on (40,435,200 visibility points x 2 correlations, 8192^2 grid, 128 w-planes,
 supports 9..65, oversampling 8).  With N > 1 ranks every rank runs the same-sized shard (weak scaling; payload
@@ -166,6 +166,7 @@ def run_ours(args):
     import torch
     import torch.distributed as dist
     from paper_2508_17187_b200 import binding as B
+    from paper_2508_17187_b200 import sharding
 
     rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -205,9 +206,7 @@ def run_ours(args):
         e[1].record()
         B.lra_grid(plan, d_vis, d_wt, d_tau, grid, sumwt)
         e[2].record()
-        if world > 1:
-            dist.all_reduce(torch.view_as_real(grid))
-            dist.all_reduce(sumwt)
+        sharding.reduce_grid(grid, sumwt)          # no-op on one GPU; one NCCL all-reduce over NVLink otherwise
         e[3].record()
         B.lra_degrid(plan, grid, d_tau, d_vis, res)
         e[4].record()
@@ -292,10 +291,18 @@ def run_ours(args):
         grid_taps = sum_s2 * ngrids
         grid_flops = grid_taps * 8.0
         achieved = grid_flops / (med["grid"] * 1e-3) / 1e12
-        roofline = {"bound": "alu", "kernel": "lra_grid (tiled register-accumulating gridder, all launches of one call)",
-                    "achieved": achieved, "peak": FP32_PEAK_TFLOPS_NOMINAL, "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS_NOMINAL,
-                    "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 flop x 1965 MHz (MEASURED_PEAKS.json has no FP32 entry)",
+        try:
+            fma_peak = B.lra_diag_fma_tflops(local)       # FMA-only microbenchmark on this GPU, outside the timed region
+            peak_src = ("measured on this GPU by lra_diag_fma_tflops (FP32 FMA-only kernel); nominal 148 SM x 128 lanes x 2 x "
+                        "1965 MHz = %.2f; MEASURED_PEAKS.json has no FP32 entry" % FP32_PEAK_TFLOPS_NOMINAL)
+        except Exception:
+            fma_peak, peak_src = FP32_PEAK_TFLOPS_NOMINAL, "derived: 148 SM x 128 FP32 lanes x 2 flop x 1965 MHz"
+        roofline = {"bound": "alu", "kernel": "lra_grid_region_kernel (all per-support-class launches of one lra_grid call, "
+                                              "CUDA events on the plan's stream around the call)",
+                    "achieved": achieved, "peak": fma_peak, "unit": "TFLOP/s", "frac": achieved / fma_peak,
+                    "peak_source": peak_src,
                     "traffic": None, "tap_updates_per_launch": grid_taps, "tap_updates_per_s": grid_taps / (med["grid"] * 1e-3),
+                    "degrid_frac": (grid_flops / (med["degrid"] * 1e-3) / 1e12 / fma_peak) if med["degrid"] else None,
                     "degrid_tap_updates_per_s": grid_taps / (med["degrid"] * 1e-3) if med["degrid"] else None,
                     "hbm_gbs_measured_peak": None if not peaks else peaks.get("hbm_gbs")}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

@@ -266,3 +266,77 @@ def test_p4_exact_patch_in_fp32(B):
         assert np.count_nonzero(g) == np.count_nonzero(expect) and sw[0, 0] == 1.0
     finally:
         run.close()
+
+
+# ---------------------------------------------------------------------------------------------------
+# Full size: the configuration bench.py times (cfg3, W-projection, 40.4 M points on 8192^2 x 2), in the same launch
+# configuration, checked on outputs the oracle computes one by one (grid_pixels / degrid_points) and, for the bin,
+# against the oracle's full bit-exact result.
+# ---------------------------------------------------------------------------------------------------
+def test_full_size_cfg3_sampled_parity(B, ref):
+    wl = W.make_workload(W.full_config(3))
+    c = wl.cfg
+    rp = ref.plan_for(wl, sort_mode=1)
+    run = run_for(B, wl, tile=c.tile, tile_x=c.tile_x)
+    try:
+        want_bin = rp.bin(wl.uvw, wl.freq, wl.cf_index)
+        assert_bin_equal(run.export(), want_bin)
+        del want_bin
+        got, sw = run.grid(wl.vis, wl.wt, None)
+        rng = np.random.default_rng(33)
+        mag = np.abs(got[0, 0])
+        scale = float(np.abs(got).max())
+        # pixels: the strongest ones, random ones among the occupied, and a few empty ones
+        flat = np.argsort(mag.ravel())[-16:]
+        occ = np.flatnonzero(mag.ravel() > 0)
+        flat = np.concatenate([flat, rng.choice(occ, 40, replace=False), rng.integers(0, mag.size, 8)])
+        pix = np.stack([np.zeros_like(flat), rng.integers(0, c.ncorr, len(flat)), flat // c.nx, flat % c.nx], 1).astype(np.int32)
+        want = rp.grid_pixels(wl.uvw, wl.freq, wl.cf_index, wl.vis, wl.wt, None, pix)
+        g = got[pix[:, 0], pix[:, 1], pix[:, 2], pix[:, 3]].astype(np.complex128)
+        assert np.abs(want).max() > 0
+        assert np.linalg.norm(g - want) <= 1e-5 * np.linalg.norm(want), np.linalg.norm(g - want) / np.linalg.norm(want)
+        assert np.abs(g - want).max() <= 1e-4 * scale
+        want_sw = wl.wt.astype(np.float64).sum(axis=(0, 1))       # every cfg3 point is valid (checked by the bin above)
+        assert np.abs(sw[0] - want_sw).max() <= 1e-6 * want_sw.max()
+        # degridding of that grid with the fused residual, on sampled points
+        res = run.degrid(got, None, vis_in=wl.vis)
+        sel = np.sort(rng.choice(c.npoints, 200, replace=False))
+        want_v = rp.degrid_points(wl.uvw, wl.freq, wl.cf_index, got, None, wl.vis, sel)
+        gv = res.reshape(-1, c.ncorr)[sel].astype(np.complex128)
+        vscale = float(np.abs(res).max())
+        assert np.linalg.norm(gv - want_v) <= 1e-5 * np.linalg.norm(want_v)
+        assert np.abs(gv - want_v).max() <= 1e-4 * vscale
+    finally:
+        run.close()
+
+
+def test_full_size_cfg1_all_outputs(B, ref):
+    """Config 1 at full size is small enough for an element-by-element comparison."""
+    wl = W.make_workload(W.full_config(1))
+    rp = ref.plan_for(wl, sort_mode=1)
+    run = run_for(B, wl, tile=wl.cfg.tile, tile_x=wl.cfg.tile_x)
+    try:
+        assert_bin_equal(run.export(), rp.bin(wl.uvw, wl.freq, wl.cf_index))
+        want, want_sw = rp.grid(wl.uvw, wl.freq, wl.cf_index, wl.vis, wl.wt, wl.tau)
+        got, sw = run.grid(wl.vis, wl.wt, wl.tau)
+        assert_close(got, want, "cfg1 full grid")
+        want_v = rp.degrid(wl.uvw, wl.freq, wl.cf_index, got.astype(np.complex128), wl.tau, vis_in=wl.vis)
+        assert_close(run.degrid(got, wl.tau, vis_in=wl.vis), want_v, "cfg1 full degrid")
+    finally:
+        run.close()
+
+
+def test_degrid_variants_agree(B, ref):
+    """Variant 1 (warp per point, the 'before' kernel and the fallback for oversized regions) against the oracle."""
+    wl = W.make_workload(W.small_config(4))
+    rng = np.random.default_rng(77)
+    c = wl.cfg
+    g = (rng.standard_normal((c.nterms, c.ncorr, c.ny, c.nx)) + 1j * rng.standard_normal((c.nterms, c.ncorr, c.ny, c.nx))).astype(np.complex64)
+    want = ref_for(ref, wl).degrid(wl.uvw, wl.freq, wl.cf_index, g.astype(np.complex128), wl.tau, vis_in=wl.vis)
+    run = run_for(B, wl)
+    try:
+        for variant in (0, 1):
+            B.lra_set_variant(run.plan, 0, variant)
+            assert_close(run.degrid(g, wl.tau, vis_in=wl.vis), want, f"degrid variant {variant}")
+    finally:
+        run.close()
