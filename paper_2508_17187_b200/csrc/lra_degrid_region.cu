@@ -15,6 +15,66 @@
 // -> caller order scatter.
 #include "lra_region.cuh"
 
+// GP (1, 2 or 4) points of a batch against the region in registers: per-lane partial sums, then a transposing
+// butterfly after which lane l holds the warp total of value l % V (V = GP x NG x (re, im)), then one shared-memory
+// atomic per value into the slot.  `left` (< GP only for GP = 4: 3 points) is the number of points that exist.
+template <int NW, int KS, int NG, int GP>
+__device__ __forceinline__ void lra_degrid_points(const lra_u64 (&gre)[KS][NG], const lra_u64 (&gim)[KS][NG],
+                                                  const unsigned char* base, int im_off, const uint4* pv, unsigned left,
+                                                  float* out, int lane, int debug) {
+  constexpr int V = 2 * NG * GP;
+  float v[V];
+#pragma unroll
+  for (int u = 0; u < GP; ++u) {
+    lra_u64 are[NG], aia[NG], aib[NG];
+#pragma unroll
+    for (int g = 0; g < NG; ++g) are[g] = aia[g] = aib[g] = 0ull;
+    const uint32_t word = pv[GP == 4 && u == 3 && left < 4 ? 2 : u].x;   // a missing 4th point repeats the 3rd ...
+    const float* re = reinterpret_cast<const float*>(base + word);
+    const float* im = reinterpret_cast<const float*>(base + word + im_off);
+#pragma unroll
+    for (int s = 0; s < KS; ++s) {
+      const lra_u64 cre = lra_pack2(re[s * 64 * NW], re[s * 64 * NW + 32]);
+      const lra_u64 cim = lra_pack2(im[s * 64 * NW], im[s * 64 * NW + 32]);
+#pragma unroll
+      for (int g = 0; g < NG; ++g) {   // conj(c) * G = (cre*Gre + cim*Gim) + i (cre*Gim - cim*Gre)
+        are[g] = lra_fma2(cre, gre[s][g], are[g]);
+        are[g] = lra_fma2(cim, gim[s][g], are[g]);
+        aia[g] = lra_fma2(cre, gim[s][g], aia[g]);
+        aib[g] = lra_fma2(cim, gre[s][g], aib[g]);
+      }
+    }
+#pragma unroll
+    for (int g = 0; g < NG; ++g) {
+      float r0, r1, a0, a1, b0, b1;
+      lra_unpack2(are[g], r0, r1);
+      lra_unpack2(aia[g], a0, a1);
+      lra_unpack2(aib[g], b0, b1);
+      v[(u * NG + g) * 2 + 0] = r0 + r1;
+      v[(u * NG + g) * 2 + 1] = (a0 + a1) - (b0 + b1);
+    }
+  }
+  if (debug == -1) {   // measurement aid: no reduction
+    float t = 0.f;
+#pragma unroll
+    for (int i = 0; i < V; ++i) t += v[i];
+    if (t == 123.456f) out[lane] = t;
+    return;
+  }
+#pragma unroll
+  for (int w = 1, n = V; n > 1; w <<= 1, n >>= 1) {
+    const bool up = (lane & w) != 0;
+#pragma unroll
+    for (int i = 0; i < n / 2; ++i) {
+      const float keep = up ? v[2 * i + 1] : v[2 * i], send = up ? v[2 * i] : v[2 * i + 1];
+      v[i] = keep + __shfl_xor_sync(0xffffffffu, send, w);
+    }
+  }
+#pragma unroll
+  for (int w = V; w < 32; w <<= 1) v[0] += __shfl_xor_sync(0xffffffffu, v[0], w);
+  if (lane < V && (unsigned)(lane / (2 * NG)) < left) atomicAdd(out + lane, v[0]);   // ... and is dropped here
+}
+
 template <int NW, int KS, int NG>
 __global__ void __launch_bounds__((NW + 1) * 32, lra_ctas_per_sm(NW, KS)) lra_degrid_region_kernel(const lra_region_args a) {
   extern __shared__ __align__(128) unsigned char smem[];
@@ -32,13 +92,12 @@ __global__ void __launch_bounds__((NW + 1) * 32, lra_ctas_per_sm(NW, KS)) lra_de
   uint32_t slot = 0, par = 0;
   const int lane_off = a.slab0 + 4 * (64 * warp + lane);
   const int im_off = a.stride_bytes;
-  constexpr int V = 8 * NG;           // values reduced together: 4 points x NG grids x (re, im)
   for (;;) {
     lra_mbar_wait(full0 + 8 * slot, par);
     unsigned char* sp = smem + LRA_RING_HDR + (size_t)slot * a.slot_bytes;
     const uint4 h = *reinterpret_cast<const uint4*>(sp);
-    const unsigned count = h.y & 0xff;
-    if (fresh && count) {
+    const unsigned count = a.debug >= 1 ? 0u : (h.y & 0xff);
+    if (fresh && (count || a.debug == 5)) {
       // ---- the item's region of the model grid, once ----
       const int hh = (a.S - 1) >> 1;
       const int ty = (int)(h.w / (unsigned)a.ntx), tx = (int)(h.w - (unsigned)ty * a.ntx);
@@ -59,8 +118,8 @@ __global__ void __launch_bounds__((NW + 1) * 32, lra_ctas_per_sm(NW, KS)) lra_de
         }
 #pragma unroll
         for (int g = 0; g < NG; ++g) {
-          gre[s][g] = lra_pack2(v[0][g].x, v[1][g].x);
-          gim[s][g] = lra_pack2(v[0][g].y, v[1][g].y);
+          gre[s][g] = lra_pack2_keep(v[0][g].x, v[1][g].x);
+          gim[s][g] = lra_pack2_keep(v[0][g].y, v[1][g].y);
         }
       }
       fresh = false;
@@ -69,52 +128,10 @@ __global__ void __launch_bounds__((NW + 1) * 32, lra_ctas_per_sm(NW, KS)) lra_de
     const uint4* pv = reinterpret_cast<const uint4*>(sp + LRA_SLOT_VAL);
     float* out = reinterpret_cast<float*>(sp + a.out_off);
     for (unsigned q0 = 0; q0 < count; q0 += 4) {
-      float v[V];
-#pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        lra_u64 are[NG], aia[NG], aib[NG];
-#pragma unroll
-        for (int g = 0; g < NG; ++g) are[g] = aia[g] = aib[g] = 0ull;
-        if (q0 + u < count) {
-          const uint32_t word = pv[q0 + u].x;
-          const float* re = reinterpret_cast<const float*>(base + word);
-          const float* im = reinterpret_cast<const float*>(base + word + im_off);
-#pragma unroll
-          for (int s = 0; s < KS; ++s) {
-            const lra_u64 cre = lra_pack2(re[s * 64 * NW], re[s * 64 * NW + 32]);
-            const lra_u64 cim = lra_pack2(im[s * 64 * NW], im[s * 64 * NW + 32]);
-#pragma unroll
-            for (int g = 0; g < NG; ++g) {   // conj(c) * G = (cre*Gre + cim*Gim) + i (cre*Gim - cim*Gre)
-              are[g] = lra_fma2(cre, gre[s][g], are[g]);
-              are[g] = lra_fma2(cim, gim[s][g], are[g]);
-              aia[g] = lra_fma2(cre, gim[s][g], aia[g]);
-              aib[g] = lra_fma2(cim, gre[s][g], aib[g]);
-            }
-          }
-        }
-#pragma unroll
-        for (int g = 0; g < NG; ++g) {
-          float r0, r1, a0, a1, b0, b1;
-          lra_unpack2(are[g], r0, r1);
-          lra_unpack2(aia[g], a0, a1);
-          lra_unpack2(aib[g], b0, b1);
-          v[(u * NG + g) * 2 + 0] = r0 + r1;
-          v[(u * NG + g) * 2 + 1] = (a0 + a1) - (b0 + b1);
-        }
-      }
-      // ---- transposing butterfly: afterwards lane l holds the warp total of value l % V ----
-#pragma unroll
-      for (int w = 1, n = V; n > 1; w <<= 1, n >>= 1) {
-        const bool up = (lane & w) != 0;
-#pragma unroll
-        for (int i = 0; i < n / 2; ++i) {
-          const float keep = up ? v[2 * i + 1] : v[2 * i], send = up ? v[2 * i] : v[2 * i + 1];
-          v[i] = keep + __shfl_xor_sync(0xffffffffu, send, w);
-        }
-      }
-#pragma unroll
-      for (int w = V; w < 32; w <<= 1) v[0] += __shfl_xor_sync(0xffffffffu, v[0], w);
-      if (lane < V && q0 + (unsigned)(lane / (2 * NG)) < count) atomicAdd(out + q0 * (2 * NG) + lane, v[0]);
+      const unsigned left = count - q0;
+      if (left >= 3) lra_degrid_points<NW, KS, NG, 4>(gre, gim, base, im_off, pv + q0, left, out + q0 * (2 * NG), lane, a.debug);
+      else if (left == 2) lra_degrid_points<NW, KS, NG, 2>(gre, gim, base, im_off, pv + q0, left, out + q0 * (2 * NG), lane, a.debug);
+      else lra_degrid_points<NW, KS, NG, 1>(gre, gim, base, im_off, pv + q0, left, out + q0 * (2 * NG), lane, a.debug);
     }
     __syncwarp();
     if (lane == 0) lra_mbar_arrive(empty0 + 8 * slot);
@@ -224,7 +241,8 @@ int lra_degrid_region_launch(lra_plan* p, const float2* grid, const float* tau, 
   a.prep = reinterpret_cast<const float*>(p->pw);   // 16 bytes per point: the slab offset word
   a.plane = (long long)p->nx * p->ny;
   a.nx = p->nx; a.ny = p->ny; a.tile_x = p->tile_x; a.tile_y = p->tile; a.ntx = p->ntx;
-  a.debug = 0;
+  const char* dbg = getenv("LRA_DEBUG_DEGRID");
+  a.debug = dbg ? atoi(dbg) : 0;
   LRA_CUDA(p, cudaEventRecord(p->ev_fork, p->stream));
   for (int s = 0; s < LRA_NAUX; ++s) LRA_CUDA(p, cudaStreamWaitEvent(p->aux[s], p->ev_fork, 0));
   int ticket = 0, turn = 0;

@@ -9,6 +9,9 @@
 #define LRA_RUNMAX 4       // points of one slab run inside a batch (longer runs are cut and load their slab again)
 #define LRA_BATCH_SLABS 12 // slab runs per batch at most
 #define LRA_BATCH_POINTS (LRA_RUNMAX * LRA_BATCH_SLABS)
+#ifndef LRA_SLOTS_TARGET
+#define LRA_SLOTS_TARGET 2   // ring slots per CTA the batch size is chosen for
+#endif
 #define LRA_KSMAX 9        // steps per consumer warp at most: 9 * 2 pixels * 2 grids * (re, im) = 72 accumulators
 
 typedef unsigned long long lra_u64;
@@ -50,7 +53,7 @@ __host__ __device__ inline lra_geom lra_make_geom(int S, int tile_x, int tile_y)
   q.stride = q.core + q.gap;
   q.per_batch = 1;
   if (q.group < LRA_NGROUP - 1) {   // a third of the CTA's shared memory per slot: 384 bytes of values + a slab per run
-    const int r = ((lra_cta_smem(q.nw, q.ks) - 512) / 3 - 256 - 4 * q.gap) / (LRA_RUNMAX * 64 + 8 * q.stride);
+    const int r = ((lra_cta_smem(q.nw, q.ks) - 512) / LRA_SLOTS_TARGET - 256 - 4 * q.gap) / (LRA_RUNMAX * 64 + 8 * q.stride);
     q.per_batch = r < 1 ? 1 : r > LRA_BATCH_SLABS ? LRA_BATCH_SLABS : r;
   }
   return q;
@@ -103,11 +106,11 @@ __device__ __forceinline__ void lra_mbar_wait(uint32_t bar, uint32_t parity) {
       "{\n"
       ".reg .pred p;\n"
       "WAIT_%=:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n"
       "@p bra DONE_%=;\n"
       "bra WAIT_%=;\n"
       "DONE_%=:\n"
-      "}\n" ::"r"(bar), "r"(parity) : "memory");
+      "}\n" ::"r"(bar), "r"(parity), "r"(0x989680u) : "memory");   // suspend-time hint: park, do not spin
 }
 // One contiguous piece, global (L2) -> shared, completion counted in bytes on `bar`.
 __device__ __forceinline__ void lra_tma_load_1d(uint32_t smem_dst, const void* gmem_src, uint32_t bytes, uint32_t bar) {
@@ -126,6 +129,15 @@ __device__ __forceinline__ lra_u64 lra_fma2(lra_u64 a, lra_u64 b, lra_u64 c) {
 __device__ __forceinline__ lra_u64 lra_pack2(float lo, float hi) {
   lra_u64 d;
   asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(lo), "f"(hi));
+  return d;
+}
+// A pair that lives across a whole item as an FFMA2 *input*: produced by an FFMA2 (x * 1 + 0), which makes the register
+// allocator keep it in an aligned register pair instead of re-assembling it from two single registers before every use.
+__device__ __forceinline__ lra_u64 lra_pack2_keep(float lo, float hi) {
+  lra_u64 d, x, one;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(x) : "f"(lo), "f"(hi));
+  asm("mov.b64 %0, {%1, %1};" : "=l"(one) : "f"(1.0f));
+  asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(x), "l"(one), "l"(0ull));
   return d;
 }
 __device__ __forceinline__ void lra_unpack2(lra_u64 v, float& lo, float& hi) {
