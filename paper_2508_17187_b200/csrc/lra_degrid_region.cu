@@ -142,34 +142,36 @@ __global__ void __launch_bounds__((NW + 1) * 32, lra_ctas_per_sm(NW, KS)) lra_de
 }
 
 // V[k][p] = sum_t tau[c][t] * res[(t, p)][i];  vis_out[k][p] = vis_in ? vis_in[k][p] - V : V   for sorted position i
-// whose support class the region kernels handle (the others were written by the fallback kernel).
+// whose support class the region kernels handle (the others were written by the fallback kernel).  One thread per point.
 __global__ void __launch_bounds__(256)
-lra_degrid_finish_kernel(const lra_rec* __restrict__ rec, const unsigned long long* __restrict__ counters,
+lra_degrid_finish_kernel(const uint4* __restrict__ pw, const unsigned long long* __restrict__ counters,
                          const float2* __restrict__ res, const float* __restrict__ tau, const float2* vis_in,
                          float2* vis_out, int nchan, int ncorr, int nterms, long long npoints, int tile_x, int tile_y) {
-  const long long n = (long long)counters[0] * ncorr;
+  const long long n = (long long)counters[0];
   const int ng = ncorr * nterms;
-  for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n; e += (long long)gridDim.x * blockDim.x) {
-    const long long i = e / ncorr;
-    const int p = (int)(e - i * ncorr);
-    const lra_rec r = rec[i];
-    if (lra_make_geom((int)(r.w & 0xff), tile_x, tile_y).group == LRA_NGROUP - 1) continue;
-    const unsigned k = r.z;
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+    const uint4 w4 = pw[i];
+    if (lra_make_geom((int)w4.z, tile_x, tile_y).group == LRA_NGROUP - 1) continue;
+    const unsigned k = w4.y;
     const int c = (int)(k % (unsigned)nchan);
-    float vx = 0.f, vy = 0.f;
-    for (int t = 0; t < nterms; ++t) {
-      const int g = t * ncorr + p, pass = g >> 1, gl = g & 1, ngp = ng - 2 * pass >= 2 ? 2 : 1;
-      const float2 v = res[(size_t)npoints * 2 * pass + (size_t)i * ngp + gl];
-      const float tw = tau ? tau[c * nterms + t] : 1.0f;
-      vx = fmaf(tw, v.x, vx);
-      vy = fmaf(tw, v.y, vy);
+#pragma unroll
+    for (int p = 0; p < 4; ++p) {
+      if (p >= ncorr) break;
+      float vx = 0.f, vy = 0.f;
+      for (int t = 0; t < nterms; ++t) {
+        const int g = t * ncorr + p, pass = g >> 1, gl = g & 1, ngp = ng - 2 * pass >= 2 ? 2 : 1;
+        const float2 v = res[(size_t)npoints * 2 * pass + (size_t)i * ngp + gl];
+        const float tw = tau ? tau[c * nterms + t] : 1.0f;
+        vx = fmaf(tw, v.x, vx);
+        vy = fmaf(tw, v.y, vy);
+      }
+      float2 o = make_float2(vx, vy);
+      if (vis_in) {
+        const float2 vi = vis_in[(size_t)k * ncorr + p];
+        o = make_float2(vi.x - vx, vi.y - vy);
+      }
+      vis_out[(size_t)k * ncorr + p] = o;
     }
-    float2 o = make_float2(vx, vy);
-    if (vis_in) {
-      const float2 vi = vis_in[(size_t)k * ncorr + p];
-      o = make_float2(vi.x - vx, vi.y - vy);
-    }
-    vis_out[(size_t)k * ncorr + p] = o;
   }
 }
 
@@ -264,7 +266,7 @@ int lra_degrid_region_launch(lra_plan* p, const float2* grid, const float* tau, 
     LRA_CUDA(p, cudaStreamWaitEvent(p->stream, p->ev_join[s], 0));
   }
   if (rc) return rc;
-  lra_degrid_finish_kernel<<<p->sm_count * 8, 256, 0, p->stream>>>(p->rec, p->counters, reinterpret_cast<const float2*>(p->prep),
+  lra_degrid_finish_kernel<<<p->sm_count * 8, 256, 0, p->stream>>>(p->pw, p->counters, reinterpret_cast<const float2*>(p->prep),
                                                                   tau, vis_in, vis_out, p->nchan, p->ncorr, p->nterms,
                                                                   (long long)n, p->tile_x, p->tile);
   LRA_LAUNCH_CHECK(p);

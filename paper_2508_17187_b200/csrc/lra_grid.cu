@@ -1,7 +1,7 @@
 // lra_grid.cu -- gridding G(c_ij) (Eq. 7) with the weights of Eq. 23:
 //   grid[t][p][iy+j][ix+i] += CF[cf][fy][fx][j][i] * (wt * tau_t * V),   sumwt[t][p] += wt * tau_t   [R6]
 // fp32 multiply-add, fp32 accumulation.  Kernels:
-//   lra_sumwt_kernel        : sum of weights, per-thread fp64 partials -> block tree -> one atomic per block
+//   lra_sumwt_kernel        : sum of weights for variant 1 (variant 0 sums them in lra_prepare_kernel)
 //   lra_grid_atomic_kernel  : variant 1, one CTA per visibility point, every tap a global float atomic (the
 //                             "before" design kept for profiling and as a second implementation in the tests)
 //   lra_grid_region_kernel  : variant 0 (default), lra_grid_region.cu
@@ -106,16 +106,16 @@ lra_grid_atomic_kernel(const lra_rec* __restrict__ rec, const unsigned long long
 }
 
 // defined in lra_grid_region.cu
-int lra_grid_region_launch(lra_plan* p, const float2* vis, const float* wt, const float* tau, float2* grid);
+int lra_grid_region_launch(lra_plan* p, const float2* vis, const float* wt, const float* tau, float2* grid, double* sumwt);
 
 int lra_grid_impl(lra_plan* p, const float2* vis, const float* wt, const float* tau, float2* grid, double* sumwt) {
   if (p->npoints == 0) return LRA_OK;
-  if (sumwt) {
+  const bool all_atomic = p->grid_variant == 1;
+  if (sumwt && all_atomic) {   // variant 0 sums the weights in lra_prepare_kernel
     lra_sumwt_kernel<<<p->sm_count * 4, 256, 0, p->stream>>>(p->rec, p->counters, wt, tau, p->nchan, p->ncorr,
                                                             p->nterms, sumwt);
     LRA_LAUNCH_CHECK(p);
   }
-  const bool all_atomic = p->grid_variant == 1;
   bool fallback = false;
   for (int c = 0; c < LRA_NCLASS; ++c)
     if (p->n_items[c] > 0 && lra_make_geom(2 * c + 1, p->tile_x, p->tile).group == LRA_NGROUP - 1) fallback = true;
@@ -126,5 +126,5 @@ int lra_grid_impl(lra_plan* p, const float2* vis, const float* wt, const float* 
     LRA_LAUNCH_CHECK(p);
     if (all_atomic) return LRA_OK;
   }
-  return lra_grid_region_launch(p, vis, wt, tau, grid);
+  return lra_grid_region_launch(p, vis, wt, tau, grid, sumwt);
 }

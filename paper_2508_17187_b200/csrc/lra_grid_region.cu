@@ -30,29 +30,67 @@
 
 // wt * tau * V of every sorted point in the form the FFMA2s consume (reading R6: (wt*tau)*V in fp32):
 //   grid g = t*ncorr + p belongs to pass g/2; a pass holds [position][gl][8] = (vx, vx, vy, vy, -vy, -vy, pw, 0)
-// with pw (lra_pipe.cuh) in the record of the pass's first grid.
+// with pw (lra_pipe.cuh) in the record of the pass's first grid.  One thread per point; the same pass over the
+// weights also gives sumwt[t][p] += wt*tau (fp64 partials per thread, block tree, one atomic per block and grid).
 __global__ void __launch_bounds__(256)
-lra_prepare_kernel(const lra_rec* __restrict__ rec, const unsigned long long* __restrict__ counters,
-                   const uint4* __restrict__ pw, const float2* __restrict__ vis, const float* __restrict__ wt,
-                   const float* __restrict__ tau, int nchan, int ncorr, int nterms, long long npoints,
-                   float4* __restrict__ prep) {
-  const long long n = (long long)counters[0] * ncorr;
+lra_prepare_kernel(const unsigned long long* __restrict__ counters, const uint4* __restrict__ pw,
+                   const float2* __restrict__ vis, const float* __restrict__ wt, const float* __restrict__ tau,
+                   int nchan, int ncorr, int nterms, long long npoints, float4* __restrict__ prep,
+                   double* __restrict__ sumwt, int fast2) {
+  const long long n = (long long)counters[0];
   const int ng = ncorr * nterms;
-  for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n; e += (long long)gridDim.x * blockDim.x) {
-    const long long i = e / ncorr;
-    const int p = (int)(e - i * ncorr);
-    const unsigned k = rec[i].z;
-    const float2 v = vis[(size_t)k * ncorr + p];
-    const float w = wt[(size_t)k * ncorr + p];
-    const float word = __uint_as_float(pw[i].x);
+  double acc[16];
+#pragma unroll
+  for (int g = 0; g < 16; ++g) acc[g] = 0.0;
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+    const uint4 w4 = pw[i];
+    const unsigned k = w4.y;
+    const float word = __uint_as_float(w4.x);
     const int c = (int)(k % (unsigned)nchan);
-    for (int t = 0; t < nterms; ++t) {
-      const float wgt = w * (tau ? tau[c * nterms + t] : 1.0f);
-      const float vx = wgt * v.x, vy = wgt * v.y;
-      const int g = t * ncorr + p, pass = g >> 1, gl = g & 1, ngp = ng - 2 * pass >= 2 ? 2 : 1;
-      float4* dst = prep + ((size_t)npoints * 2 * pass + (size_t)i * ngp + gl) * 2;
-      dst[0] = make_float4(vx, vx, vy, vy);
-      dst[1] = make_float4(-vy, -vy, word, 0.f);
+    float2 v[4];
+    float w[4];
+    if (fast2) {   // two correlations, 16-byte aligned vis: one load each
+      const float4 vv = *reinterpret_cast<const float4*>(vis + (size_t)k * 2);
+      const float2 ww = *reinterpret_cast<const float2*>(wt + (size_t)k * 2);
+      v[0] = make_float2(vv.x, vv.y); v[1] = make_float2(vv.z, vv.w); w[0] = ww.x; w[1] = ww.y;
+    } else {
+#pragma unroll
+      for (int p = 0; p < 4; ++p)
+        if (p < ncorr) { v[p] = vis[(size_t)k * ncorr + p]; w[p] = wt[(size_t)k * ncorr + p]; }
+    }
+#pragma unroll
+    for (int t = 0; t < 4; ++t) {
+      if (t >= nterms) break;
+      const float tw = tau ? tau[c * nterms + t] : 1.0f;
+#pragma unroll
+      for (int p = 0; p < 4; ++p) {
+        if (p >= ncorr) break;
+        const float wgt = w[p] * tw;
+        acc[t * 4 + p] += (double)wgt;
+        const float vx = wgt * v[p].x, vy = wgt * v[p].y;
+        const int g = t * ncorr + p, pass = g >> 1, gl = g & 1, ngp = ng - 2 * pass >= 2 ? 2 : 1;
+        float4* dst = prep + ((size_t)npoints * 2 * pass + (size_t)i * ngp + gl) * 2;
+        dst[0] = make_float4(vx, vx, vy, vy);
+        dst[1] = make_float4(-vy, -vy, word, 0.f);
+      }
+    }
+  }
+  if (!sumwt) return;
+  __shared__ double sh[8][16];
+  const int l = threadIdx.x & 31, wp = threadIdx.x >> 5;
+#pragma unroll
+  for (int g = 0; g < 16; ++g) {
+    double x = acc[g];
+    for (int o = 16; o > 0; o >>= 1) x += __shfl_down_sync(0xffffffffu, x, o);
+    if (l == 0) sh[wp][g] = x;
+  }
+  __syncthreads();
+  if (threadIdx.x < 16) {
+    const int t = threadIdx.x >> 2, pp = threadIdx.x & 3;
+    if (t < nterms && pp < ncorr) {
+      double x = 0.0;
+      for (int ww = 0; ww < 8; ++ww) x += sh[ww][threadIdx.x];
+      atomicAdd(&sumwt[t * ncorr + pp], x);
     }
   }
 }
@@ -200,7 +238,7 @@ static int lra_launch_class_nw(lra_plan* p, const lra_region_args& a, const lra_
   }
 }
 
-int lra_grid_region_launch(lra_plan* p, const float2* vis, const float* wt, const float* tau, float2* grid) {
+int lra_grid_region_launch(lra_plan* p, const float2* vis, const float* wt, const float* tau, float2* grid, double* sumwt) {
   const int ng = p->ncorr * p->nterms;
   const int64_t n = p->npoints;
   int rc = LRA_OK;
@@ -212,8 +250,9 @@ int lra_grid_region_launch(lra_plan* p, const float2* vis, const float* wt, cons
     LRA_CUDA(p, cudaMalloc(&p->prep, (size_t)need * sizeof(float)));
     p->prep_capacity = need;
   }
-  lra_prepare_kernel<<<p->sm_count * 8, 256, 0, p->stream>>>(p->rec, p->counters, p->pw, vis, wt, tau, p->nchan, p->ncorr,
-                                                            p->nterms, (long long)n, (float4*)p->prep);
+  lra_prepare_kernel<<<p->sm_count * 8, 256, 0, p->stream>>>(p->counters, p->pw, vis, wt, tau, p->nchan, p->ncorr, p->nterms,
+                                                            (long long)n, (float4*)p->prep, sumwt,
+                                                            p->ncorr == 2 && ((uintptr_t)vis & 15) == 0 && ((uintptr_t)wt & 7) == 0);
   LRA_LAUNCH_CHECK(p);
   LRA_CUDA(p, cudaMemsetAsync(p->counters + LRA_TICKET0, 0, LRA_NTICKET * sizeof(unsigned long long), p->stream));
   lra_region_args a;

@@ -12,6 +12,9 @@
 #ifndef LRA_SLOTS_TARGET
 #define LRA_SLOTS_TARGET 2   // ring slots per CTA the batch size is chosen for
 #endif
+#ifndef LRA_CTA_CAP
+#define LRA_CTA_CAP 6      // CTAs per SM at most
+#endif
 #define LRA_KSMAX 9        // steps per consumer warp at most: 9 * 2 pixels * 2 grids * (re, im) = 72 accumulators
 
 typedef unsigned long long lra_u64;
@@ -32,11 +35,14 @@ struct lra_geom {
   int gap, stride;                // floats of zeros between planes; stride = core + gap
   int per_batch;                  // slab runs per batch
 };
-__host__ __device__ constexpr int lra_ks_max(int nw) { return nw == 8 ? 6 : LRA_KSMAX; }
+#ifndef LRA_KSLIM
+#define LRA_KSLIM 9
+#endif
+__host__ __device__ constexpr int lra_ks_max(int nw) { return nw == 16 ? LRA_KSMAX : nw == 8 ? (LRA_KSLIM < 6 ? LRA_KSLIM : 6) : LRA_KSLIM; }
 // CTAs per SM the (NW, KS) kernel is built for: ~12 registers per step (8 accumulators, 4 taps in flight) + 36.
 __host__ __device__ constexpr int lra_ctas_per_sm(int nw, int ks) {
   const int regs = (12 * ks + 36 + 7) / 8 * 8, r = 65536 / ((nw + 1) * 32 * regs);
-  return r < 1 ? 1 : r > 6 ? 6 : r;
+  return r < 1 ? 1 : r > LRA_CTA_CAP ? LRA_CTA_CAP : r;
 }
 // Shared memory of a CTA and of one ring slot (3 slots per CTA at least, whenever a slab fits).
 __host__ __device__ constexpr int lra_cta_smem(int nw, int ks) { return (227 * 1024) / lra_ctas_per_sm(nw, ks) - 1024; }

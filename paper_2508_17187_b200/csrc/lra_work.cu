@@ -14,7 +14,7 @@ struct lra_work_args {
   int shift_x, shift_y, ntx, tile_x, tile_y;
   uint4* work;
   uint32_t* batch;     // 16 words per batch
-  uint4* pw;           // one 16-byte record per sorted position, the word in .x
+  uint4* pw;           // one 16-byte record per sorted position: {word, k, S, 0}
 };
 
 // exclusive prefix sum over the block (256 threads); returns the block total through `total`
@@ -179,7 +179,7 @@ __global__ void __launch_bounds__(256) lra_work_kernel(const lra_work_args a) {
       const unsigned r = (j - item_first_run[it]) % (unsigned)q.per_batch;
       const int ix = rc[e].x & 0xffff, iy = rc[e].x >> 16;
       const int ox = ix - ((ix >> a.shift_x) << a.shift_x), oy = iy - ((iy >> a.shift_y) << a.shift_y);
-      a.pw[i] = make_uint4((unsigned)(4 * (q.gap + (int)r * 2 * q.stride - (oy * q.rx + ox))), rc[e].z, 0u, 0u);
+      a.pw[i] = make_uint4((unsigned)(4 * (q.gap + (int)r * 2 * q.stride - (oy * q.rx + ox))), rc[e].z, rc[e].w & 0xffu, 0u);
     }
   }
 }
