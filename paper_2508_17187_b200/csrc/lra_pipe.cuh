@@ -61,6 +61,8 @@ __host__ __device__ inline lra_geom lra_make_geom(int S, int tile_x, int tile_y)
   if (q.group < LRA_NGROUP - 1) {   // a third of the CTA's shared memory per slot: 384 bytes of values + a slab per run
     const int r = ((lra_cta_smem(q.nw, q.ks) - 512) / LRA_SLOTS_TARGET - 256 - 4 * q.gap) / (LRA_RUNMAX * 64 + 8 * q.stride);
     q.per_batch = r < 1 ? 1 : r > LRA_BATCH_SLABS ? LRA_BATCH_SLABS : r;
+    // even one slab per slot must fit the CTA's shared memory (values + record + ring header: 1 KB), else fall back
+    if (4 * (q.gap + 2 * q.stride) + 1024 > lra_cta_smem(q.nw, q.ks)) { q.group = LRA_NGROUP - 1; q.per_batch = 1; }
   }
   return q;
 }
