@@ -32,7 +32,8 @@ lra_index_kernel(lra_index_args a, const double* __restrict__ uvw, const double*
                  const double* __restrict__ sv, const int32_t* __restrict__ cf_index,
                  const int32_t* __restrict__ cf_support, int32_t* __restrict__ ix_o, int32_t* __restrict__ iy_o,
                  int8_t* __restrict__ fx_o, int8_t* __restrict__ fy_o, uint64_t* __restrict__ key_o,
-                 uint64_t* __restrict__ skey_o, uint32_t* __restrict__ sval_o, unsigned long long* __restrict__ counters) {
+                 uint64_t* __restrict__ skey_o, uint32_t* __restrict__ sval_o, unsigned long long* __restrict__ counters,
+                 const int64_t* __restrict__ slab_off, lra_rec* __restrict__ urec) {
   long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x;
   unsigned long long nvalid = 0, s2 = 0;
   if (k < a.npoints) {
@@ -63,6 +64,11 @@ lra_index_kernel(lra_index_args a, const double* __restrict__ uvw, const double*
     }
     ix_o[k] = ix; iy_o[k] = iy; fx_o[k] = (int8_t)fx; fy_o[k] = (int8_t)fy; key_o[k] = key;
     skey_o[k] = skey; sval_o[k] = (uint32_t)k;
+    if (ok) {   // the record the gridder / degridder consume (lra_internal.cuh), gathered into sorted order later
+      const int phase = (fy + a.os / 2) * a.os + (fx + a.os / 2);
+      const long long off = slab_off[cf] + (long long)phase * (2 * lra_plane_floats(S, a.tile_x));
+      urec[k] = make_uint4((uint32_t)ix | ((uint32_t)iy << 16), (uint32_t)(off >> 2), (uint32_t)k, (uint32_t)S | ((uint32_t)cf << 8));
+    }
   }
   // block totals -> two atomics per block
   __shared__ unsigned long long sh[2][8];
@@ -183,27 +189,13 @@ lra_tile_start_kernel(const uint64_t* __restrict__ sorted_keys, long long n, uns
   for (long long q = t_prev + 1; q <= t_here; ++q) tile_start[q] = (uint32_t)i;
 }
 
-// Sorted records for the gridder / degridder: one 16-byte record per sorted position (see lra_internal.cuh).
+// Sorted records for the gridder / degridder: one 16-byte gather per sorted position (see lra_internal.cuh).
 __global__ void __launch_bounds__(256)
 lra_record_kernel(const uint32_t* __restrict__ perm, const unsigned long long* __restrict__ counters,
-                  const int32_t* __restrict__ ix, const int32_t* __restrict__ iy, const int8_t* __restrict__ fx,
-                  const int8_t* __restrict__ fy, const int32_t* __restrict__ cf_index,
-                  const int32_t* __restrict__ cf_support, const int64_t* __restrict__ slab_off, int os,
-                  int tile_x, lra_rec* __restrict__ rec) {
+                  const lra_rec* __restrict__ urec, lra_rec* __restrict__ rec) {
   long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
   if (i >= (long long)counters[0]) return;
-  uint32_t k = perm[i];
-  int cf = cf_index ? cf_index[k] : 0;
-  int S = cf_support[cf];
-  int stride = 2 * lra_plane_floats(S, tile_x);
-  int phase = (fy[k] + os / 2) * os + (fx[k] + os / 2);
-  long long off = slab_off[cf] + (long long)phase * stride;
-  lra_rec r;
-  r.x = (uint32_t)ix[k] | ((uint32_t)iy[k] << 16);
-  r.y = (uint32_t)(off >> 2);
-  r.z = k;
-  r.w = (uint32_t)S | ((uint32_t)cf << 8);
-  rec[i] = r;
+  rec[i] = urec[perm[i]];
 }
 
 template <typename T>
@@ -230,6 +222,7 @@ int lra_bin_impl(lra_plan* p, int64_t nrow, int32_t nchan, const double* uvw, co
       if ((rc = lra_regrow(p, &p->sval[b], n))) return rc;
     }
     if ((rc = lra_regrow(p, &p->rec, n))) return rc;
+    if ((rc = lra_regrow(p, &p->urec, n))) return rc;
     p->capacity = n;
   }
   if (nchan > p->su_capacity) {
@@ -254,6 +247,7 @@ int lra_bin_impl(lra_plan* p, int64_t nrow, int32_t nchan, const double* uvw, co
   if (p->sort_mode == LRA_SORT_TILE_CF) per_tile = (unsigned long long)p->n_cf * p->os * p->os;
   const unsigned long long invalid_key = (unsigned long long)p->ntiles * per_tile;
   p->nrow = nrow; p->nchan = nchan; p->npoints = n;
+  p->per_tile = per_tile; p->tile_start_done = false;   // per-tile offsets are computed by lra_bin_export on demand
   p->sorted_buf = 0;
   if (n > 0) {
     lra_index_args a;
@@ -261,7 +255,8 @@ int lra_bin_impl(lra_plan* p, int64_t nrow, int32_t nchan, const double* uvw, co
     a.sort_mode = p->sort_mode; a.n_cf = p->n_cf; a.nchan = nchan; a.npoints = n; a.invalid_sort_key = invalid_key;
     int blocks = (int)((n + 255) / 256);
     lra_index_kernel<<<blocks, 256, 0, p->stream>>>(a, uvw, p->d_su, p->d_sv, cf_index, p->d_cf_support, p->ix, p->iy,
-                                                    p->fx, p->fy, p->key, p->skey[0], p->sval[0], p->counters);
+                                                    p->fx, p->fy, p->key, p->skey[0], p->sval[0], p->counters, p->d_slab_off,
+                                                    p->urec);
     LRA_LAUNCH_CHECK(p);
     // radix passes over the bits of invalid_key (the largest sort key)
     int nbits = 0;
@@ -292,11 +287,7 @@ int lra_bin_impl(lra_plan* p, int64_t nrow, int32_t nchan, const double* uvw, co
       cur ^= 1;
     }
     p->sorted_buf = cur;
-    lra_tile_start_kernel<<<(int)((n + 1 + 255) / 256), 256, 0, p->stream>>>(p->skey[cur], n, per_tile, p->ntiles,
-                                                                             p->tile_start);
-    LRA_LAUNCH_CHECK(p);
-    lra_record_kernel<<<blocks, 256, 0, p->stream>>>(p->sval[cur], p->counters, p->ix, p->iy, p->fx, p->fy, cf_index,
-                                                     p->d_cf_support, p->d_slab_off, p->os, p->tile_x, p->rec);
+    lra_record_kernel<<<blocks, 256, 0, p->stream>>>(p->sval[cur], p->counters, p->urec, p->rec);
     LRA_LAUNCH_CHECK(p);
     if ((rc = lra_build_work(p))) return rc;
   } else {
@@ -321,8 +312,19 @@ extern "C" int lra_bin_export(lra_plan* p, int32_t* ix, int32_t* iy, int8_t* fx,
     if (key) LRA_CUDA(p, cudaMemcpyAsync(key, p->key, n * 8, k, p->stream));
     if (perm) LRA_CUDA(p, cudaMemcpyAsync(perm, p->sval[p->sorted_buf], n * 4, k, p->stream));
   }
-  if (tile_start)
+  if (tile_start) {
+    if (!p->tile_start_done) {
+      if (n) {
+        lra_tile_start_kernel<<<(int)((n + 1 + 255) / 256), 256, 0, p->stream>>>(p->skey[p->sorted_buf], (long long)n, p->per_tile,
+                                                                                 p->ntiles, p->tile_start);
+        LRA_LAUNCH_CHECK(p);
+      } else {
+        LRA_CUDA(p, cudaMemsetAsync(p->tile_start, 0, (size_t)(p->ntiles + 1) * sizeof(uint32_t), p->stream));
+      }
+      p->tile_start_done = true;
+    }
     LRA_CUDA(p, cudaMemcpyAsync(tile_start, p->tile_start, (size_t)(p->ntiles + 1) * 4, k, p->stream));
+  }
   unsigned long long nv = 0;
   LRA_CUDA(p, cudaMemcpyAsync(&nv, p->counters, sizeof nv, cudaMemcpyDeviceToHost, p->stream));
   LRA_CUDA(p, cudaStreamSynchronize(p->stream));

@@ -48,7 +48,10 @@ struct lra_plan {
   int sorted_buf;
   uint32_t* hist;           // radix histograms
   int64_t hist_capacity;
-  uint32_t* tile_start;     // [ntiles + 1]
+  uint32_t* tile_start;     // [ntiles + 1]; filled on demand by lra_bin_export (nothing else reads it)
+  bool tile_start_done;
+  unsigned long long per_tile;   // keys per tile of the last lra_bin
+  lra_rec* urec;            // [npoints] the records in caller order (written by the index kernel)
   lra_rec* rec;             // [npoints] sorted records (first n_valid meaningful)
   unsigned long long* counters;  // see lra_pipe.cuh
   double *d_su, *d_sv;      // per-channel scale tables
