@@ -38,9 +38,10 @@ struct lra_geom {
 #ifndef LRA_KSLIM
 #define LRA_KSLIM 9
 #endif
-__host__ __device__ constexpr int lra_ks_max(int nw) { return nw == 16 ? LRA_KSMAX : nw == 8 ? (LRA_KSLIM < 6 ? LRA_KSLIM : 6) : LRA_KSLIM; }
+__host__ __device__ constexpr int lra_ks_max(int nw) { return nw == 16 ? LRA_KSMAX : nw == 8 ? (LRA_KSLIM < 7 ? LRA_KSLIM : 7) : LRA_KSLIM; }
 // CTAs per SM the (NW, KS) kernel is built for: ~12 registers per step (8 accumulators, 4 taps in flight) + 36.
 __host__ __device__ constexpr int lra_ctas_per_sm(int nw, int ks) {
+  if (nw == 8 && ks == 7) return 2;   // 112 registers: measured without spills
   const int regs = (12 * ks + 36 + 7) / 8 * 8, r = 65536 / ((nw + 1) * 32 * regs);
   return r < 1 ? 1 : r > LRA_CTA_CAP ? LRA_CTA_CAP : r;
 }
