@@ -30,6 +30,7 @@ sys.path.insert(0, ROOT)
 from paper_2508_17187_b200 import workloads as W  # noqa: E402
 
 FP32_PEAK_TFLOPS_NOMINAL = 148 * 128 * 2 * 1.965e9 / 1e12   # 148 SMs x 128 FP32 lanes x 2 flop x 1965 MHz
+NCU_DRAM_BYTES_GRID_CFG3 = 4.313e9   # measured once under ncu, see profiles/r1_c_summary.md ("DRAM and L2 traffic")
 METRIC = "visibility points per second through bin+grid+degrid"
 UNIT = "vis_points/s"
 
@@ -301,7 +302,10 @@ def run_ours(args):
                                               "CUDA events on the plan's stream around the call)",
                     "achieved": achieved, "peak": fma_peak, "unit": "TFLOP/s", "frac": achieved / fma_peak,
                     "peak_source": peak_src,
-                    "traffic": None, "tap_updates_per_launch": grid_taps, "tap_updates_per_s": grid_taps / (med["grid"] * 1e-3),
+                    "traffic": NCU_DRAM_BYTES_GRID_CFG3 if (cfg.cfg_id == 3 and not args.small and not args.tile) else None,
+                    "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum over the 29 lra_grid_region_kernel launches of one "
+                                      "lra_grid call, profiles/r1_c_summary.md (ncu, cfg3); algorithmic bytes 2.37e9",
+                    "tap_updates_per_launch": grid_taps, "tap_updates_per_s": grid_taps / (med["grid"] * 1e-3),
                     "degrid_frac": (grid_flops / (med["degrid"] * 1e-3) / 1e12 / fma_peak) if med["degrid"] else None,
                     "degrid_tap_updates_per_s": grid_taps / (med["degrid"] * 1e-3) if med["degrid"] else None,
                     "hbm_gbs_measured_peak": None if not peaks else peaks.get("hbm_gbs")}
