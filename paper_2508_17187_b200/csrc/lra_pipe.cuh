@@ -6,14 +6,14 @@
 #include "lra_internal.cuh"
 
 #define LRA_CHUNK 1024     // sorted positions per work-list chunk = upper bound on the points of one work item
-#define LRA_RUNMAX 4       // points of one slab run inside a batch (longer runs are cut and load their slab again)
+#define LRA_RUNMAX 16      // points of one slab run inside a batch (longer runs are cut and load their slab again)
 #define LRA_BATCH_SLABS 12 // slab runs per batch at most
 #define LRA_BATCH_POINTS (LRA_RUNMAX * LRA_BATCH_SLABS)
 #ifndef LRA_SLOTS_TARGET
 #define LRA_SLOTS_TARGET 2   // ring slots per CTA the batch size is chosen for
 #endif
 #ifndef LRA_CTA_CAP
-#define LRA_CTA_CAP 6      // CTAs per SM at most
+#define LRA_CTA_CAP 10      // CTAs per SM at most
 #endif
 #define LRA_KSMAX 9        // steps per consumer warp at most: 9 * 2 pixels * 2 grids * (re, im) = 72 accumulators
 
