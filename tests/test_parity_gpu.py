@@ -273,41 +273,63 @@ def test_p4_exact_patch_in_fp32(B):
 # configuration, checked on outputs the oracle computes one by one (grid_pixels / degrid_points) and, for the bin,
 # against the oracle's full bit-exact result.
 # ---------------------------------------------------------------------------------------------------
-def test_full_size_cfg3_sampled_parity(B, ref):
-    wl = W.make_workload(W.full_config(3))
+def _full_size_sampled(B, ref, n, check_bin=True, npix=64, npts=200):
+    """Full-size configuration n in bench.py's launch configuration: bin bit-exact (optional), gridded pixels and
+    degridded residuals compared with the oracle's one-by-one values (grid_pixels / degrid_points)."""
+    wl = W.make_workload(W.full_config(n))
     c = wl.cfg
     rp = ref.plan_for(wl, sort_mode=1)
     run = run_for(B, wl, tile=c.tile, tile_x=c.tile_x)
     try:
-        want_bin = rp.bin(wl.uvw, wl.freq, wl.cf_index)
-        assert_bin_equal(run.export(), want_bin)
-        del want_bin
-        got, sw = run.grid(wl.vis, wl.wt, None)
-        rng = np.random.default_rng(33)
-        mag = np.abs(got[0, 0])
+        if check_bin:
+            want_bin = rp.bin(wl.uvw, wl.freq, wl.cf_index)
+            assert_bin_equal(run.export(), want_bin)
+            del want_bin
+        got, sw = run.grid(wl.vis, wl.wt, wl.tau)
+        rng = np.random.default_rng(33 + n)
         scale = float(np.abs(got).max())
-        # pixels: the strongest ones, random ones among the occupied, and a few empty ones
-        flat = np.argsort(mag.ravel())[-16:]
-        occ = np.flatnonzero(mag.ravel() > 0)
-        flat = np.concatenate([flat, rng.choice(occ, 40, replace=False), rng.integers(0, mag.size, 8)])
-        pix = np.stack([np.zeros_like(flat), rng.integers(0, c.ncorr, len(flat)), flat // c.nx, flat % c.nx], 1).astype(np.int32)
-        want = rp.grid_pixels(wl.uvw, wl.freq, wl.cf_index, wl.vis, wl.wt, None, pix)
+        nsel = np.array([npix // 4, npix - npix // 4 - 8, 8])
+        pix = []
+        for t in range(c.nterms):                      # strongest, random occupied and a few random pixels of some grids
+            p_ = int(rng.integers(0, c.ncorr))
+            mag = np.abs(got[t, p_]).ravel()
+            flat = np.concatenate([np.argsort(mag)[-nsel[0]:], rng.choice(np.flatnonzero(mag > 0), nsel[1], replace=False),
+                                   rng.integers(0, mag.size, nsel[2])])
+            pix.append(np.stack([np.full_like(flat, t), np.full_like(flat, p_), flat // c.nx, flat % c.nx], 1))
+        pix = np.concatenate(pix).astype(np.int32)
+        want = rp.grid_pixels(wl.uvw, wl.freq, wl.cf_index, wl.vis, wl.wt, wl.tau, pix)
         g = got[pix[:, 0], pix[:, 1], pix[:, 2], pix[:, 3]].astype(np.complex128)
         assert np.abs(want).max() > 0
         assert np.linalg.norm(g - want) <= 1e-5 * np.linalg.norm(want), np.linalg.norm(g - want) / np.linalg.norm(want)
         assert np.abs(g - want).max() <= 1e-4 * scale
-        want_sw = wl.wt.astype(np.float64).sum(axis=(0, 1))       # every cfg3 point is valid (checked by the bin above)
-        assert np.abs(sw[0] - want_sw).max() <= 1e-6 * want_sw.max()
+        nv, _ = B.lra_tap_count(run.plan)
+        if nv == c.npoints:                            # every point valid: sumwt is the plain sum of wt * tau
+            tau = np.ones((c.nchan, c.nterms)) if wl.tau is None else wl.tau.astype(np.float64)
+            want_sw = np.einsum("rcp,ct->tp", wl.wt.astype(np.float64), tau)
+            assert np.abs(sw - want_sw).max() <= 1e-6 * np.abs(want_sw).max()
         # degridding of that grid with the fused residual, on sampled points
-        res = run.degrid(got, None, vis_in=wl.vis)
-        sel = np.sort(rng.choice(c.npoints, 200, replace=False))
-        want_v = rp.degrid_points(wl.uvw, wl.freq, wl.cf_index, got, None, wl.vis, sel)
+        res = run.degrid(got, wl.tau, vis_in=wl.vis)
+        sel = np.sort(rng.choice(c.npoints, npts, replace=False))
+        want_v = rp.degrid_points(wl.uvw, wl.freq, wl.cf_index, got, wl.tau, wl.vis, sel)
         gv = res.reshape(-1, c.ncorr)[sel].astype(np.complex128)
-        vscale = float(np.abs(res).max())
         assert np.linalg.norm(gv - want_v) <= 1e-5 * np.linalg.norm(want_v)
-        assert np.abs(gv - want_v).max() <= 1e-4 * vscale
+        assert np.abs(gv - want_v).max() <= 1e-4 * float(np.abs(res).max())
     finally:
         run.close()
+
+
+def test_full_size_cfg3_sampled_parity(B, ref):
+    _full_size_sampled(B, ref, 3)
+
+
+@pytest.mark.parametrize("n", [4, 5])
+def test_full_size_cfg4_cfg5_sampled_parity(B, ref, n):
+    _full_size_sampled(B, ref, n)
+
+
+def test_full_size_cfg2_sampled_parity(B, ref):
+    """323 M points: the oracle's full bin (a single-threaded merge sort) is left to the smaller configurations."""
+    _full_size_sampled(B, ref, 2, check_bin=False, npix=32, npts=100)
 
 
 def test_full_size_cfg1_all_outputs(B, ref):
