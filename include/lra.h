@@ -74,8 +74,9 @@ int lra_plan_create(lra_plan** out, const lra_plan_desc* desc);
 int lra_plan_destroy(lra_plan* p);
 
 /* Re-ordering: for every visibility point computes grid pixel (ix, iy), sub-pixel phase
- * (fx, fy), validity [R2, R4] and the sort key [R5], then stable-sorts the valid point indices by key and
- * records per-tile start offsets.  The result stays in the plan and is consumed by lra_grid / lra_degrid.
+ * (fx, fy), validity [R2, R4] and the sort key [R5], then stable-sorts the valid point indices by key (the
+ * per-tile start offsets follow from the sorted keys and are produced when lra_bin_export asks for them).  The result
+ * stays in the plan and is consumed by lra_grid / lra_degrid.
  *   nrow, nchan : npoints = nrow*nchan must be < 2^31
  *   uvw_m       : device double [nrow][3], baseline coordinates in metres
  *   freq_hz     : HOST double [nchan]  (small; the per-channel scale (freq/c)*scale is formed on the host)

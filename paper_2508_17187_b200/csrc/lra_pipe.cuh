@@ -1,6 +1,7 @@
-// lra_pipe.cuh -- pieces shared by the strip gridder and the strip degridder: PTX wrappers (mbarrier, 1-D TMA bulk
-// copy, packed fp32x2 FMA, vector reductions to global memory), the kernel configurations ("groups") and the
-// format of the stage stream that lra_work.cu builds and the kernels consume.
+// lra_pipe.cuh -- pieces shared by lra_work.cu, the region gridder and the region degridder: the geometry of a support
+// class (consumer warps, steps, shared-memory layout of a slab), the format of the batch stream that lra_work.cu
+// builds and the kernels consume, and PTX wrappers (mbarrier, 1-D TMA bulk copy, packed fp32x2 FMA, vector reductions
+// to global memory).
 // Product code: shares nothing with oracle/.
 #pragma once
 #include "lra_internal.cuh"
@@ -25,7 +26,8 @@ typedef unsigned long long lra_u64;
 // e / (64*NW), lane e % 32, half (e / 32) % 2, i.e. at step s a warp owns the 64 consecutive pixels that start at
 // 64*(NW*s + warp) and a lane owns two of them, 32 apart (the two halves of one FFMA2).  NW = 2, 4, 8 or 16 is the
 // smallest for which ks = ceil(RX*RY / (64*NW)) <= lra_ks_max(NW) (the register budget that still leaves two CTAs of
-// NW = 8 on an SM); a region too large for NW = 16 goes to the fallback kernels (global atomics).  Every lane reads a tap for every point, at linear slab index e - off with
+// NW = 8 on an SM); a region too large for NW = 16 goes to the fallback kernels (global atomics).  Every lane reads a
+// tap for every point, at linear slab index e - off with
 // off = oy*RX + ox <= pre, so a slab plane sits in shared memory between zeros: `gap` floats before (>= pre) and
 // after (>= the pixels past the last tap) -- consecutive planes share a gap, which no copy ever writes.
 // ---------------------------------------------------------------------------------------------------
@@ -78,8 +80,9 @@ __host__ __device__ inline int lra_class_of(int S) { return (S - 1) >> 1; }
 //   batch = per_batch consecutive runs of one item: what occupies one slot of a CTA's shared-memory ring.
 //           64 bytes: uint4 {first sorted position, count | flags, runs, tile id}, then the slab offsets of its
 //           runs in 16-byte units (uint32 x 12).  LRA_BATCH_LAST marks the last batch of its item.
-//   pw    = for every sorted position 16 bytes (one TMA granule), first word: the byte offset, inside the slot's slab area, of the float the
-//           lane that owns pixel 0 of the region reads for this point: 4 * (gap + run * 2 * stride - (oy*RX + ox)).
+//   pw    = for every sorted position 16 bytes (one TMA granule) {word, k, S, 0}; word = the byte offset, inside the
+//           slot's slab area, of the float the lane that owns pixel 0 of the region reads for this point:
+//           4 * (gap + run * 2 * stride - (oy*RX + ox)).
 // ---------------------------------------------------------------------------------------------------
 #define LRA_BATCH_LAST 0x40000000u
 #define LRA_BATCH_END 0x80000000u
