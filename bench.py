@@ -250,40 +250,79 @@ def run_ours(args):
     # ---- end to end through the C ABI with HOST buffers: H2D of the step's inputs + D2H of its results ----
     e2e = None
     if not args.no_e2e:
+        # Software-pipelined over the steps, the way a caller streams data through the C ABI: two sets of device inputs and
+        # outputs; the H2D copy of step i+1 (copy stream) and the D2H read of step i-1 (read-back stream) run beside the
+        # kernels of step i (plan's stream).  Every step still copies all of its inputs in and all of its results out.
+        k = max(2, min(args.steps, 8))
+        cur = torch.cuda.current_stream()
+        s_in, s_out = torch.cuda.Stream(), torch.cuda.Stream()
+        sets = []
+        for _ in range(2):
+            sets.append({"uvw": torch.empty_like(d_uvw), "cfi": None if d_cfi is None else torch.empty_like(d_cfi),
+                         "vis": torch.empty_like(d_vis), "wt": torch.empty_like(d_wt), "grid": torch.empty_like(grid),
+                         "sumwt": torch.empty_like(sumwt), "res": torch.empty_like(res),
+                         "in_ready": None, "computed": None, "read_back": None})
         h_grid = torch.empty(grid.shape, dtype=torch.complex64).pin_memory()
         h_res = torch.empty(res.shape, dtype=torch.complex64).pin_memory()
         h_sw = torch.empty(sumwt.shape, dtype=torch.float64).pin_memory()
 
-        def e2e_step():
-            d_uvw.copy_(h_uvw, non_blocking=True)
-            if d_cfi is not None:
-                d_cfi.copy_(h_cfi, non_blocking=True)
-            d_vis.copy_(h_vis, non_blocking=True)
-            d_wt.copy_(h_wt, non_blocking=True)
-            step(False)
-            h_grid.copy_(grid, non_blocking=True)
-            h_res.copy_(res, non_blocking=True)
-            h_sw.copy_(sumwt, non_blocking=True)
+        def upload(b):
+            with torch.cuda.stream(s_in):
+                if b["computed"] is not None:
+                    s_in.wait_event(b["computed"])          # the previous user of this input set has finished
+                b["uvw"].copy_(h_uvw, non_blocking=True)
+                if b["cfi"] is not None:
+                    b["cfi"].copy_(h_cfi, non_blocking=True)
+                b["vis"].copy_(h_vis, non_blocking=True)
+                b["wt"].copy_(h_wt, non_blocking=True)
+                b["in_ready"] = s_in.record_event()
 
-        e2e_step()
+        def compute(b):
+            cur.wait_event(b["in_ready"])
+            if b["read_back"] is not None:
+                cur.wait_event(b["read_back"])              # its outputs of two steps ago have been read
+            b["grid"].zero_()
+            b["sumwt"].zero_()
+            B.lra_bin(plan, b["uvw"], wl.freq, b["cfi"])
+            B.lra_grid(plan, b["vis"], b["wt"], d_tau, b["grid"], b["sumwt"])
+            sharding.reduce_grid(b["grid"], b["sumwt"])
+            B.lra_degrid(plan, b["grid"], d_tau, b["vis"], b["res"])
+            b["computed"] = cur.record_event()
+
+        def read_back(b):
+            with torch.cuda.stream(s_out):
+                s_out.wait_event(b["computed"])
+                h_grid.copy_(b["grid"], non_blocking=True)
+                h_res.copy_(b["res"], non_blocking=True)
+                h_sw.copy_(b["sumwt"], non_blocking=True)
+                b["read_back"] = s_out.record_event()
+
+        def e2e_run(nsteps):
+            upload(sets[0])
+            for i in range(nsteps):
+                if i + 1 < nsteps:
+                    upload(sets[(i + 1) % 2])
+                compute(sets[i % 2])
+                read_back(sets[i % 2])
+
+        e2e_run(2)
         sync_all()
-        k = max(1, min(args.steps, 3))
+        for b in sets:
+            b["in_ready"] = b["computed"] = b["read_back"] = None
         t0 = time.perf_counter()
-        a, b = ev(), ev()
-        a.record()
-        for _ in range(k):
-            e2e_step()
-        b.record()
+        e2e_run(k)
         sync_all()
-        e_ms = max(a.elapsed_time(b), (time.perf_counter() - t0) * 1e3) / k
+        e_ms = (time.perf_counter() - t0) * 1e3 / k         # wall clock around k pipelined steps, all streams drained
         if world > 1:
             t = torch.tensor([e_ms], dtype=torch.float64, device="cuda")
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             e_ms = float(t.item())
         h2d = h_uvw.numel() * 8 + (0 if h_cfi is None else h_cfi.numel() * 4) + h_vis.numel() * 8 + h_wt.numel() * 4
         d2h = h_grid.numel() * 8 + h_res.numel() * 8 + h_sw.numel() * 8
-        e2e = {"value": cfg.npoints * world / (e_ms * 1e-3), "unit": UNIT, "ms_per_step": e_ms,
-               "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)}
+        e2e = {"value": cfg.npoints * world / (e_ms * 1e-3), "unit": UNIT, "ms_per_step": e_ms, "steps": k,
+               "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+               "how": "k steps software-pipelined over two buffer sets: H2D of step i+1 and D2H of step i-1 overlap the kernels "
+                      "of step i; wall clock around the k steps with every stream drained"}
 
     if rank == 0:
         peaks = measured_peaks()
