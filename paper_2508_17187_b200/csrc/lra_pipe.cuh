@@ -16,6 +16,9 @@
 #ifndef LRA_CTA_CAP
 #define LRA_CTA_CAP 10      // CTAs per SM at most
 #endif
+#ifndef LRA_REGS_PER_STEP
+#define LRA_REGS_PER_STEP 12   // 8 accumulators + 4 taps in flight per step; 10 (one more CTA per SM) measured no faster
+#endif
 #define LRA_KSMAX 9        // steps per consumer warp at most: 9 * 2 pixels * 2 grids * (re, im) = 72 accumulators
 
 typedef unsigned long long lra_u64;
@@ -44,7 +47,7 @@ __host__ __device__ constexpr int lra_ks_max(int nw) { return nw == 16 ? LRA_KSM
 // CTAs per SM the (NW, KS) kernel is built for: ~12 registers per step (8 accumulators, 4 taps in flight) + 36.
 __host__ __device__ constexpr int lra_ctas_per_sm(int nw, int ks) {
   if (nw == 8 && ks == 7) return 2;   // 112 registers: measured without spills
-  const int regs = (12 * ks + 36 + 7) / 8 * 8, r = 65536 / ((nw + 1) * 32 * regs);
+  const int regs = (LRA_REGS_PER_STEP * ks + 36 + 7) / 8 * 8, r = 65536 / ((nw + 1) * 32 * regs);
   return r < 1 ? 1 : r > LRA_CTA_CAP ? LRA_CTA_CAP : r;
 }
 // Shared memory of a CTA and of one ring slot (3 slots per CTA at least, whenever a slab fits).
