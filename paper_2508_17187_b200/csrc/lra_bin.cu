@@ -212,6 +212,7 @@ int lra_bin_impl(lra_plan* p, int64_t nrow, int32_t nchan, const double* uvw, co
   int rc;
   if (n > p->capacity) {
     LRA_CUDA(p, cudaStreamSynchronize(p->stream));
+    p->capacity = 0;   // a failure part-way leaves freed (null) arrays behind: the next call must grow again
     if ((rc = lra_regrow(p, &p->ix, n))) return rc;
     if ((rc = lra_regrow(p, &p->iy, n))) return rc;
     if ((rc = lra_regrow(p, &p->fx, n))) return rc;
@@ -227,6 +228,7 @@ int lra_bin_impl(lra_plan* p, int64_t nrow, int32_t nchan, const double* uvw, co
   }
   if (nchan > p->su_capacity) {
     LRA_CUDA(p, cudaStreamSynchronize(p->stream));
+    p->su_capacity = 0;
     if ((rc = lra_regrow(p, &p->d_su, nchan))) return rc;
     if ((rc = lra_regrow(p, &p->d_sv, nchan))) return rc;
     p->su_capacity = nchan;
@@ -271,6 +273,7 @@ int lra_bin_impl(lra_plan* p, int64_t nrow, int32_t nchan, const double* uvw, co
     int64_t hist_n = (int64_t)LRA_RADIX * sblocks;
     if (hist_n > p->hist_capacity) {
       LRA_CUDA(p, cudaStreamSynchronize(p->stream));
+      p->hist_capacity = 0;
       if ((rc = lra_regrow(p, &p->hist, hist_n))) return rc;
       p->hist_capacity = hist_n;
     }

@@ -21,7 +21,7 @@
 template <int NW, int KS, int NG, int GP>
 __device__ __forceinline__ void lra_degrid_points(const lra_u64 (&gre)[KS][NG], const lra_u64 (&gim)[KS][NG],
                                                   const unsigned char* base, int im_off, const uint4* pv, unsigned left,
-                                                  float* out, int lane, int debug) {
+                                                  float* out, int lane) {
   constexpr int V = 2 * NG * GP;
   float v[V];
 #pragma unroll
@@ -53,13 +53,6 @@ __device__ __forceinline__ void lra_degrid_points(const lra_u64 (&gre)[KS][NG], 
       v[(u * NG + g) * 2 + 0] = r0 + r1;
       v[(u * NG + g) * 2 + 1] = (a0 + a1) - (b0 + b1);
     }
-  }
-  if (debug == -1) {   // measurement aid: no reduction
-    float t = 0.f;
-#pragma unroll
-    for (int i = 0; i < V; ++i) t += v[i];
-    if (t == 123.456f) out[lane] = t;
-    return;
   }
 #pragma unroll
   for (int w = 1, n = V; n > 1; w <<= 1, n >>= 1) {
@@ -96,8 +89,8 @@ __global__ void __launch_bounds__((NW + 1) * 32, lra_ctas_per_sm(NW, KS)) lra_de
     lra_mbar_wait(full0 + 8 * slot, par);
     unsigned char* sp = smem + LRA_RING_HDR + (size_t)slot * a.slot_bytes;
     const uint4 h = *reinterpret_cast<const uint4*>(sp);
-    const unsigned count = a.debug >= 1 ? 0u : (h.y & 0xff);
-    if (fresh && (count || a.debug == 5)) {
+    const unsigned count = h.y & 0xff;
+    if (fresh && count) {
       // ---- the item's region of the model grid, once ----
       const int hh = (a.S - 1) >> 1;
       const int ty = (int)(h.w / (unsigned)a.ntx), tx = (int)(h.w - (unsigned)ty * a.ntx);
@@ -129,9 +122,9 @@ __global__ void __launch_bounds__((NW + 1) * 32, lra_ctas_per_sm(NW, KS)) lra_de
     float* out = reinterpret_cast<float*>(sp + a.out_off);
     for (unsigned q0 = 0; q0 < count; q0 += 4) {
       const unsigned left = count - q0;
-      if (left >= 3) lra_degrid_points<NW, KS, NG, 4>(gre, gim, base, im_off, pv + q0, left, out + q0 * (2 * NG), lane, a.debug);
-      else if (left == 2) lra_degrid_points<NW, KS, NG, 2>(gre, gim, base, im_off, pv + q0, left, out + q0 * (2 * NG), lane, a.debug);
-      else lra_degrid_points<NW, KS, NG, 1>(gre, gim, base, im_off, pv + q0, left, out + q0 * (2 * NG), lane, a.debug);
+      if (left >= 3) lra_degrid_points<NW, KS, NG, 4>(gre, gim, base, im_off, pv + q0, left, out + q0 * (2 * NG), lane);
+      else if (left == 2) lra_degrid_points<NW, KS, NG, 2>(gre, gim, base, im_off, pv + q0, left, out + q0 * (2 * NG), lane);
+      else lra_degrid_points<NW, KS, NG, 1>(gre, gim, base, im_off, pv + q0, left, out + q0 * (2 * NG), lane);
     }
     __syncwarp();
     if (lane == 0) lra_mbar_arrive(empty0 + 8 * slot);
@@ -181,7 +174,11 @@ static int lra_degrid_launch_class(lra_plan* p, lra_region_args a, const lra_geo
   int smem = 0;
   if (!lra_region_ring(q, 16 + 8 * NG, &a, &smem)) return LRA_EINVAL;
   auto kern = lra_degrid_region_kernel<NW, KS, NG>;
-  LRA_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  static int attr_smem[LRA_MAX_DEVICES];   // per instantiation and device: the opt-in is made once, not per launch
+  if (p->device < 0 || p->device >= LRA_MAX_DEVICES || attr_smem[p->device] < smem) {
+    LRA_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    if (p->device >= 0 && p->device < LRA_MAX_DEVICES) attr_smem[p->device] = smem;
+  }
   a.work = p->work + p->item_off[c];
   a.n_items = (unsigned)p->n_items[c];
   a.batch = reinterpret_cast<const uint4*>(p->batch) + (size_t)p->batch_off[c] * 4;
@@ -243,8 +240,6 @@ int lra_degrid_region_launch(lra_plan* p, const float2* grid, const float* tau, 
   a.prep = reinterpret_cast<const float*>(p->pw);   // 16 bytes per point: the slab offset word
   a.plane = (long long)p->nx * p->ny;
   a.nx = p->nx; a.ny = p->ny; a.tile_x = p->tile_x; a.tile_y = p->tile; a.ntx = p->ntx;
-  const char* dbg = getenv("LRA_DEBUG_DEGRID");
-  a.debug = dbg ? atoi(dbg) : 0;
   LRA_CUDA(p, cudaEventRecord(p->ev_fork, p->stream));
   for (int s = 0; s < LRA_NAUX; ++s) LRA_CUDA(p, cudaStreamWaitEvent(p->aux[s], p->ev_fork, 0));
   int ticket = 0, turn = 0;

@@ -135,7 +135,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, lra_ctas_per_sm(NW, KS)) lra_gr
     lra_mbar_wait(full0 + 8 * slot, par);
     const unsigned char* sp = smem + LRA_RING_HDR + (size_t)slot * a.slot_bytes;
     const uint4 h = *reinterpret_cast<const uint4*>(sp);
-    const unsigned count = a.debug >= 1 ? 0u : (h.y & 0xff);
+    const unsigned count = h.y & 0xff;
     const unsigned char* base = sp + lane_off;
     const ulonglong2* vp = reinterpret_cast<const ulonglong2*>(sp + LRA_SLOT_VAL);
     for (unsigned q = 0; q < count; ++q, vp += 2 * NG) {
@@ -154,7 +154,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, lra_ctas_per_sm(NW, KS)) lra_gr
     }
     __syncwarp();
     if (lane == 0) lra_mbar_arrive(empty0 + 8 * slot);
-    if ((h.y & LRA_BATCH_LAST) && a.debug < 4) {
+    if (h.y & LRA_BATCH_LAST) {
       // ---- row a4: add the item's region to the grid, once ----
       const int hh = (a.S - 1) >> 1;
       const int ty = (int)(h.w / (unsigned)a.ntx), tx = (int)(h.w - (unsigned)ty * a.ntx);
@@ -194,7 +194,11 @@ static int lra_launch_class(lra_plan* p, lra_region_args a, const lra_geom& q, i
   int smem = 0;
   if (!lra_region_ring(q, NG * 32, &a, &smem)) return LRA_EINVAL;
   auto kern = lra_grid_region_kernel<NW, KS, NG>;
-  LRA_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  static int attr_smem[LRA_MAX_DEVICES];   // per instantiation and device: the opt-in is made once, not per launch
+  if (p->device < 0 || p->device >= LRA_MAX_DEVICES || attr_smem[p->device] < smem) {
+    LRA_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    if (p->device >= 0 && p->device < LRA_MAX_DEVICES) attr_smem[p->device] = smem;
+  }
   a.work = p->work + p->item_off[c];
   a.n_items = (unsigned)p->n_items[c];
   a.batch = reinterpret_cast<const uint4*>(p->batch) + (size_t)p->batch_off[c] * 4;
@@ -259,8 +263,6 @@ int lra_grid_region_launch(lra_plan* p, const float2* vis, const float* wt, cons
   a.slabs = p->slabs;
   a.plane = (long long)p->nx * p->ny;
   a.nx = p->nx; a.ny = p->ny; a.tile_x = p->tile_x; a.tile_y = p->tile; a.ntx = p->ntx;
-  const char* dbg = getenv("LRA_DEBUG");
-  a.debug = dbg ? atoi(dbg) : 0;
   // the per-class launches are independent: spread them over the plan's internal streams
   LRA_CUDA(p, cudaEventRecord(p->ev_fork, p->stream));
   for (int s = 0; s < LRA_NAUX; ++s) LRA_CUDA(p, cudaStreamWaitEvent(p->aux[s], p->ev_fork, 0));

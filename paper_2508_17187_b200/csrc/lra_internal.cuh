@@ -18,6 +18,7 @@ typedef uint4 lra_rec;
 #define LRA_NGROUP 5   // kernel configurations of the region gridder / degridder; the last one is the fallback
 #define LRA_NCLASS 65  // support classes: class (S - 1) / 2 for S = 1, 3, .., 129
 #define LRA_NAUX 4     // internal streams the per-class launches of one call are spread over
+#define LRA_MAX_DEVICES 64
 
 struct lra_plan {
   // ---- descriptor (host copies) ----

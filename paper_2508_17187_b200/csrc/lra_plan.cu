@@ -3,7 +3,15 @@
 #include <new>
 #include <string.h>
 
+#include <nvtx3/nvToolsExt.h>
+
 #include "lra_pipe.cuh"
+
+// NVTX range over one ABI call (one range per call; header-only NVTX 3, a no-op without a profiler).
+struct lra_nvtx_range {
+  explicit lra_nvtx_range(const char* name) { nvtxRangePushA(name); }
+  ~lra_nvtx_range() { nvtxRangePop(); }
+};
 
 // Re-lay one oversampled kernel into phase-major planar slabs (reading R3; layout in
 // lra_internal.cuh):  tap (j + h, i + h) of slab (fyi, fxi) = K[(j*os - fy) + c0][(i*os - fx) + c0],
@@ -39,6 +47,7 @@ __global__ void lra_relayout_kernel(const float2* __restrict__ K, float* __restr
 static int is_pow2(int x) { return x > 0 && (x & (x - 1)) == 0; }
 
 extern "C" int lra_plan_create(lra_plan** out, const lra_plan_desc* d) {
+  lra_nvtx_range nvtx_("lra_plan_create");
   if (!out) return LRA_EINVAL;
   *out = nullptr;
   if (!d || d->nx < 1 || d->ny < 1 || d->nx > 32768 || d->ny > 32768) return LRA_EINVAL;
@@ -141,6 +150,7 @@ extern "C" int lra_plan_destroy(lra_plan* p) {
 
 extern "C" int lra_bin(lra_plan* p, int64_t nrow, int32_t nchan, const double* uvw_m, const double* freq_hz,
                        const int32_t* cf_index) {
+  lra_nvtx_range nvtx_("lra_bin");
   if (!p || nrow < 0 || nchan < 1 || (nrow > 0 && !uvw_m) || !freq_hz) return LRA_EINVAL;
   if (nrow * (int64_t)nchan >= ((int64_t)1 << 31)) return LRA_EINVAL;
   LRA_CUDA(p, cudaSetDevice(p->device));
@@ -148,6 +158,7 @@ extern "C" int lra_bin(lra_plan* p, int64_t nrow, int32_t nchan, const double* u
 }
 
 extern "C" int lra_grid(lra_plan* p, const void* vis, const float* wt, const float* tau, void* grid, double* sumwt) {
+  lra_nvtx_range nvtx_("lra_grid");
   if (!p) return LRA_EINVAL;
   if (!p->binned) return LRA_ESTATE;
   if (!grid || (p->npoints > 0 && (!vis || !wt))) return LRA_EINVAL;
@@ -156,6 +167,7 @@ extern "C" int lra_grid(lra_plan* p, const void* vis, const float* wt, const flo
 }
 
 extern "C" int lra_degrid(lra_plan* p, const void* grid, const float* tau, const void* vis_in, void* vis_out) {
+  lra_nvtx_range nvtx_("lra_degrid");
   if (!p) return LRA_EINVAL;
   if (!p->binned) return LRA_ESTATE;
   if (!grid || (p->npoints > 0 && !vis_out)) return LRA_EINVAL;
@@ -177,7 +189,7 @@ extern "C" int lra_tap_count(lra_plan* p, int64_t* n_valid, int64_t* sum_s2) {
 }
 
 extern "C" int lra_set_variant(lra_plan* p, int32_t grid_variant, int32_t degrid_variant) {
-  if (!p || grid_variant < 0 || grid_variant > 3 || degrid_variant < 0 || degrid_variant > 3) return LRA_EINVAL;
+  if (!p || grid_variant < 0 || grid_variant > 1 || degrid_variant < 0 || degrid_variant > 1) return LRA_EINVAL;
   p->grid_variant = grid_variant;
   p->degrid_variant = degrid_variant;
   return LRA_OK;

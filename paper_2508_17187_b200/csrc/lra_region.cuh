@@ -2,8 +2,6 @@
 // kernel arguments, the layout of a ring slot, the producer warp and the ring set-up.
 // Product code: shares nothing with oracle/.
 #pragma once
-#include <stdlib.h>
-
 #include "lra_pipe.cuh"
 
 struct lra_region_args {
@@ -21,7 +19,6 @@ struct lra_region_args {
   int nslot, slot_bytes, slab0; // ring geometry: slots, bytes per slot, offset of the slab area inside a slot
   int out_off;                  // degridder: offset of the per-point results inside a slot
   float2* res;                  // degridder: this pass's results, [sorted position][grids of the pass]
-  int debug;                    // measurement aid (LRA_DEBUG env): 1 = consumers skip the taps, 2 = no slab copies
 };
 
 // slot layout (bytes): batch record (64) | pad | prepared values | slab area.  The slab area is gap, re plane of run
@@ -75,7 +72,6 @@ __device__ __forceinline__ void lra_region_producer(const lra_region_args& a, co
         // lane 4j owns the batch: slot hand-over, record, prepared values
         const uint32_t sa = slots0 + slot * a.slot_bytes, fb = full0 + 8 * slot;
         const uint32_t nr = __shfl_sync(0xffffffffu, cur.z, 4 * j) & 0xff;
-        const bool slabs = a.debug < 2;
         if (OUTW > 0) {
           if (lane == 0) lra_mbar_wait(empty0 + 8 * slot, par ^ 1);
           __syncwarp();
@@ -85,10 +81,10 @@ __device__ __forceinline__ void lra_region_producer(const lra_region_args& a, co
         ++issued;
         if (lane == (int)(4 * j)) {
           const uint32_t count = cur.y & 0xff;
-          const bool pv = vals && a.debug < 3;
+          const bool pv = vals != nullptr;
           lra_mbar_wait(empty0 + 8 * slot, par ^ 1);
           asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(sa), "r"(cur.x), "r"(cur.y), "r"(cur.z), "r"(cur.w) : "memory");
-          lra_mbar_arrive_expect_tx(fb, (pv ? count * val_bytes : 0u) + (slabs ? nr * 2u * (uint32_t)a.core_bytes : 0u));
+          lra_mbar_arrive_expect_tx(fb, (pv ? count * val_bytes : 0u) + nr * 2u * (uint32_t)a.core_bytes);
           if (pv) lra_tma_load_1d(sa + LRA_SLOT_VAL, reinterpret_cast<const unsigned char*>(vals) + (size_t)cur.x * val_bytes, count * val_bytes, fb);
         }
         __syncwarp();   // the slot is free from here on
@@ -98,7 +94,7 @@ __device__ __forceinline__ void lra_region_producer(const lra_region_args& a, co
           const uint32_t c = r & 3;
           const uint32_t pick = c == 0 ? cur.x : c == 1 ? cur.y : c == 2 ? cur.z : cur.w;
           const uint32_t off16 = __shfl_sync(0xffffffffu, pick, 4 * j + 1 + (r >> 2));
-          if (lane == 0 && slabs) {
+          if (lane == 0) {
             const unsigned char* src_b = reinterpret_cast<const unsigned char*>(a.slabs) + ((size_t)off16 << 4);
             const uint32_t dst = sa + slab0 + a.gap_bytes + r * 2 * a.stride_bytes;
             lra_tma_load_1d(dst, src_b, a.core_bytes, fb);
@@ -152,8 +148,6 @@ static inline bool lra_region_ring(const lra_geom& q, int val_bytes, lra_region_
   int nslot = (lra_cta_smem(q.nw, q.ks) - LRA_RING_HDR) / slot_bytes;
   if (nslot < 1) return false;
   if (nslot > 4) nslot = 4;
-  const char* env = getenv("LRA_NSLOT");
-  if (env && atoi(env) >= 1 && atoi(env) < nslot) nslot = atoi(env);
   a->S = q.S; a->rx = q.rx; a->ry = q.ry; a->ks = q.ks;
   a->core_bytes = 4 * q.core; a->stride_bytes = 4 * q.stride; a->gap_bytes = 4 * q.gap;
   a->nslot = nslot; a->slot_bytes = slot_bytes; a->slab0 = slab0;

@@ -3,9 +3,6 @@
 // lra_bin).  Part of "re-ordering for runtime performance": the sorted order itself is the
 // bit-exact contract of lra_bin; this file only says how that order is cut into pieces for the CTAs.
 // Formats: lra_pipe.cuh.
-#include <stdio.h>
-#include <stdlib.h>
-
 #include "lra_pipe.cuh"
 
 struct lra_work_args {
@@ -224,15 +221,6 @@ int lra_build_work(lra_plan* p) {
     off[128 + c] = (unsigned long long)batches;
     items += p->n_items[c];
     batches += p->n_batches[c];
-  }
-  if (getenv("LRA_VERBOSE")) {
-    for (int c = 0; c < LRA_NCLASS; ++c)
-      if (p->n_items[c]) {
-        const lra_geom q = lra_make_geom(2 * c + 1, p->tile_x, p->tile);
-        fprintf(stderr, "liblra: S=%d nw=%d ks=%d per_batch=%d stride=%d gap=%d items=%lld batches=%lld\n", q.S, q.nw, q.ks,
-                q.per_batch, q.stride, q.gap, (long long)p->n_items[c], (long long)p->n_batches[c]);
-      }
-    fprintf(stderr, "liblra: %lld points, %lld items, %lld batches\n", (long long)n, (long long)items, (long long)batches);
   }
   if ((rc = lra_grow(p, &p->work, &p->work_capacity, items))) return rc;
   int64_t bwords = p->batch_capacity * 16;

@@ -98,6 +98,26 @@ def test_p2_nearest_pixel_histogram(ref):
     assert abs(sw[0, 0] - wt[ok].astype(np.float64).sum()) <= 1e-12 * sw[0, 0]
 
 
+def test_p2b_sum_of_weights_with_tau_counts_valid_points_only(ref):
+    """sumwt[t][p] = sum over the VALID points of wt * tau (R4, R6, R11): points off the grid contribute nothing, and
+    the Taylor weight multiplies the weight (dropping it, or counting invalid points, fails here)."""
+    rng = np.random.default_rng(22)
+    nx, ny, n, nchan, ncorr, nterms = 40, 36, 1500, 3, 2, 3
+    uvw, freq = pixel_problem(rng, n, nx + 10, ny + 10, nchan)     # some points fall off the grid
+    vis, wt = cn(rng, (n, nchan, ncorr)), rng.uniform(0.5, 1, (n, nchan, ncorr)).astype(np.float32)
+    tau = rng.uniform(-1, 1, (nchan, nterms)).astype(np.float32)
+    sup, off, data, _ = random_cf_table(rng, [3], 2)
+    p = ref.RefPlan(nx, ny, ncorr, nterms, 2, 1.0, 1.0, sup, off, data)
+    _, sw = p.grid(uvw, freq, None, vis, wt, tau)
+    valid = (p.bin(uvw, freq, None)["key"] != np.uint64(2 ** 64 - 1)).reshape(n, nchan)
+    assert 0 < valid.sum() < n * nchan
+    want = np.einsum("rcp,ct->tp", wt.astype(np.float64) * valid[:, :, None], tau.astype(np.float64))
+    assert np.abs(sw - want).max() <= 1e-12 * np.abs(want).max()
+    # not vacuous: without tau, or with the invalid points, the sums differ
+    assert np.abs(np.einsum("rcp,ct->tp", wt.astype(np.float64), tau.astype(np.float64)) - want).max() > 1e-3
+    assert np.abs(np.einsum("rcp->p", wt.astype(np.float64) * valid[:, :, None])[None, :] - want).max() > 1e-3
+
+
 # ---------------------------------------------------------------------------------------------------
 # P3 sum(grid) = sum_k wt*tau*V * slabsum(cf, fy, fx), slab sums straight from K_cf by strided slicing
 # ---------------------------------------------------------------------------------------------------
@@ -111,9 +131,12 @@ def test_p3_sum_of_grid(ref):
     vis, wt = cn(rng, (n, nchan, ncorr)), rng.uniform(0.5, 1, (n, nchan, ncorr)).astype(np.float32)
     tau = rng.uniform(-1, 1, (nchan, nterms)).astype(np.float32)
     p = ref.RefPlan(nx, ny, ncorr, nterms, os_, 1.0, 1.0, sup, off, data)
-    g, _ = p.grid(uvw, freq, cf_index, vis, wt, tau)
+    g, sw = p.grid(uvw, freq, cf_index, vis, wt, tau)
     b = p.bin(uvw, freq, cf_index)
     assert b["n_valid"] == n * nchan
+    # sum of weights with Taylor weights (R6, R11): sumwt[t][p] = sum_{r,c} wt[r][c][p] * tau[c][t], no CF factor
+    want_sw = np.einsum("rcp,ct->tp", wt.astype(np.float64), tau.astype(np.float64))
+    assert np.abs(sw - want_sw).max() <= 1e-12 * np.abs(want_sw).max()
     expect = np.zeros((nterms, ncorr), np.complex128)
     for k in range(n * nchan):
         r, c = divmod(k, nchan)
