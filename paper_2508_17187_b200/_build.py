@@ -1,38 +1,65 @@
-"""Builds liblra.so (the C-ABI CUDA library) in-tree with nvcc for sm_100a."""
+"""Builds liblra.so (the C-ABI CUDA library) in-tree with nvcc for sm_100a.
+
+Every csrc/*.cu is compiled to an object file under build/ (in parallel: the region kernels are templates with many
+instantiations) and the objects are linked into paper_2508_17187_b200/liblra.so.
+"""
 from __future__ import annotations
 
 import glob
 import os
 import subprocess
+from concurrent.futures import ThreadPoolExecutor
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _ROOT = os.path.dirname(_HERE)
 SO_PATH = os.path.join(_HERE, "liblra.so")
+OBJ_DIR = os.path.join(_HERE, "build")
 SOURCES = sorted(glob.glob(os.path.join(_HERE, "csrc", "*.cu")))
 HEADERS = sorted(glob.glob(os.path.join(_HERE, "csrc", "*.cuh"))) + [os.path.join(_ROOT, "include", "lra.h")]
 
-NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "--use_fast_math=false",
-              "-Xcompiler", "-fPIC,-ffp-contract=off", "-shared", "-cudart", "static"]
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
+              "-Xcompiler", "-fPIC,-ffp-contract=off"]
 
 
 def needs_build() -> bool:
     if not os.path.exists(SO_PATH):
         return True
     t = os.path.getmtime(SO_PATH)
-    return any(os.path.getmtime(f) > t for f in SOURCES + HEADERS)
+    return any(os.path.getmtime(f) > t for f in SOURCES + HEADERS + [os.path.abspath(__file__)])
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if force or needs_build():
-        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        flags = [f for f in NVCC_FLAGS if f != "--use_fast_math=false"]
-        cmd = [nvcc] + flags + (["-Xptxas", "-v"] if verbose else []) + ["-I", os.path.join(_ROOT, "include"),
-                                                                         "-I", os.path.join(_HERE, "csrc"),
-                                                                         "-o", SO_PATH] + SOURCES
-        subprocess.check_call(cmd)
+def _obj(src: str) -> str:
+    return os.path.join(OBJ_DIR, os.path.splitext(os.path.basename(src))[0] + ".o")
+
+
+def build(force: bool = False, verbose: bool = False, defines=()) -> str:
+    if not (force or needs_build()):
+        return SO_PATH
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    os.makedirs(OBJ_DIR, exist_ok=True)
+    newest_header = max(os.path.getmtime(f) for f in HEADERS + [os.path.abspath(__file__)])
+    common = NVCC_FLAGS + [f"-D{d}" for d in defines] + (["-Xptxas", "-v"] if verbose else []) + [
+        "-I", os.path.join(_ROOT, "include"), "-I", os.path.join(_HERE, "csrc")]
+
+    def compile_one(src: str):
+        obj = _obj(src)
+        if not force and os.path.exists(obj) and os.path.getmtime(obj) > max(os.path.getmtime(src), newest_header):
+            return None
+        r = subprocess.run([nvcc] + common + ["-c", src, "-o", obj], capture_output=True, text=True)
+        if r.returncode != 0:
+            raise RuntimeError(f"nvcc failed on {src}:\n{r.stdout}\n{r.stderr}")
+        return r.stderr if verbose else None
+
+    with ThreadPoolExecutor(max_workers=min(len(SOURCES), os.cpu_count() or 4)) as ex:
+        for out in ex.map(compile_one, SOURCES):
+            if out:
+                print(out)
+    subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-cudart", "static",
+                           "-o", SO_PATH] + [_obj(s) for s in SOURCES])
     return SO_PATH
 
 
 if __name__ == "__main__":
     import sys
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv,
+                defines=[a[2:] for a in sys.argv[1:] if a.startswith("-D")]))

@@ -66,7 +66,7 @@ lra_index_kernel(lra_index_args a, const double* __restrict__ uvw, const double*
     skey_o[k] = skey; sval_o[k] = (uint32_t)k;
     if (ok) {   // the record the gridder / degridder consume (lra_internal.cuh), gathered into sorted order later
       const int phase = (fy + a.os / 2) * a.os + (fx + a.os / 2);
-      const long long off = slab_off[cf] + (long long)phase * (2 * lra_plane_floats(S, a.tile_x));
+      const long long off = slab_off[cf] + (long long)phase * (2 * lra_slab_complex(S, a.tile_x));
       urec[k] = make_uint4((uint32_t)ix | ((uint32_t)iy << 16), (uint32_t)(off >> 2), (uint32_t)k, (uint32_t)S | ((uint32_t)cf << 8));
     }
   }

@@ -23,7 +23,7 @@ __global__ void __launch_bounds__(256)
 lra_degrid_warp_kernel(const lra_rec* __restrict__ rec, const unsigned long long* __restrict__ counters,
                        const float* __restrict__ slabs, const float2* __restrict__ grid, const float* __restrict__ tau,
                        const float2* vis_in, float2* vis_out, int nchan, int nterms, int nx, int ny, int tile_x, int tile_y,
-                       int only_fallback) {
+                       int ng, int only_fallback) {
   const long long n = (long long)counters[0];
   const size_t plane = (size_t)nx * ny;
   const int lane = threadIdx.x & 31;
@@ -32,9 +32,8 @@ lra_degrid_warp_kernel(const lra_rec* __restrict__ rec, const unsigned long long
   for (long long i = warp0; i < n; i += nwarps) {
     const lra_rec r = rec[i];
     const int ix = r.x & 0xffff, iy = r.x >> 16, S = r.w & 0xff, h = (S - 1) >> 1;
-    if (only_fallback && lra_make_geom(S, tile_x, tile_y).group != LRA_NGROUP - 1) continue;   // the region kernels do those
-    const float* slab = slabs + ((size_t)r.y << 2);
-    const int pf = lra_plane_floats(S, tile_x);
+    if (only_fallback && lra_make_geom(S, tile_x, tile_y, ng).nw != 0) continue;   // the region kernels do those
+    const float2* slab = reinterpret_cast<const float2*>(slabs + ((size_t)r.y << 2));
     const unsigned k = r.z;
     const int c = (int)(k % (unsigned)nchan);
     float tw[4];
@@ -46,8 +45,7 @@ lra_degrid_warp_kernel(const lra_rec* __restrict__ rec, const unsigned long long
     const float2* g0 = grid + (size_t)(iy - h) * nx + (ix - h);
     for (int j = 0; j < S; ++j) {
       for (int ii = lane; ii < S; ii += 32) {
-        const int ti = lra_tap_index(S, tile_x, j, ii);
-        const float2 cf = make_float2(slab[ti], slab[pf + ti]);
+        const float2 cf = slab[lra_tap_index(S, tile_x, j, ii)];
         const float2* gp = g0 + (size_t)j * nx + ii;
 #pragma unroll
         for (int p = 0; p < NC; ++p) {
@@ -99,13 +97,13 @@ int lra_degrid_impl(lra_plan* p, const float2* grid, const float* tau, const flo
   const bool all_warp = p->degrid_variant == 1;
   bool fallback = false;
   for (int c = 0; c < LRA_NCLASS; ++c)
-    if (p->n_items[c] > 0 && lra_make_geom(2 * c + 1, p->tile_x, p->tile).group == LRA_NGROUP - 1) fallback = true;
+    if (p->n_items[c] > 0 && lra_make_geom(2 * c + 1, p->tile_x, p->tile, p->ncorr * p->nterms).nw == 0) fallback = true;
   if (all_warp || fallback) {   // regions that fit no group of the region kernel (or the "before" variant)
     const int blocks = p->sm_count * 8;
 #define LRA_DG(NC)                                                                                                  \
   lra_degrid_warp_kernel<NC><<<blocks, 256, 0, p->stream>>>(p->rec, p->counters, p->slabs, grid, tau, vis_in, vis_out, \
                                                             p->nchan, p->nterms, p->nx, p->ny, p->tile_x, p->tile,    \
-                                                            all_warp ? 0 : 1)
+                                                            p->ncorr * p->nterms, all_warp ? 0 : 1)
     switch (p->ncorr) {
       case 1: LRA_DG(1); break;
       case 2: LRA_DG(2); break;

@@ -1,0 +1,4 @@
+// lra_degrid_region_ng2.cu -- the region degridder's kernels for passes of 2 grids (lra_degrid_region.cuh).
+#include "lra_degrid_region.cuh"
+
+template int lra_degrid_launch_ng<2>(lra_plan*, const lra_region_args&, const lra_geom&, int, cudaStream_t);

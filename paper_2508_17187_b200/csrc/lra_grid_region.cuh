@@ -1,0 +1,265 @@
+// lra_grid_region.cuh -- the default gridder (variant 0): region-owning CTAs that accumulate in REGISTERS with packed
+// fp32x2 FMAs and read the convolution function from a TMA-fed shared-memory ring.  Kernel template and its launch
+// dispatch; instantiated per number of grids in lra_grid_region_ng*.cu, driven by lra_grid_region.cu.
+//
+// Operation: Eq. 7 / Eq. 23 of arxiv 2508.17187, tap loop of SURVEY Sec. 8(a) rows a3, a4.
+//
+// Design (B200-first; the paper's Kokkos kernel is prior art only):
+//   * lra_bin left the visibility points sorted by uv tile (8 x 8 pixels by default), then by CF slab.  A work item
+//     (lra_work.cu) is a run of at most LRA_CHUNK points of one tile and one support S; persistent CTAs take items
+//     through an atomic ticket, so the dense centre of a VLA-like uv plane is spread over many CTAs.
+//   * A CTA owns the item's region = tile + halo, RX x RY = (tile_x + S - 1) x (tile + S - 1) pixels, numbered
+//     linearly e = y*RX + x.  Consumer warp w owns, at step s, the 64 consecutive pixels from 64*(NW*s + w); a lane
+//     owns two of them, 32 apart.  The complex accumulator of a pixel is one aligned register pair per grid, kept for
+//     the whole item and added to the HBM grid once per item with red.global.add.v2.f32 (row a4).
+//   * The CF slab is stored with the region's pitch RX as interleaved complex taps with zeros ending each row
+//     (lra_internal.cuh), so the tap of pixel e for a point whose footprint starts at linear pixel `off` is simply
+//     slab[e - off]: one 8-byte shared-memory load per lane and pixel, 32 consecutive values per warp (no bank
+//     conflicts whatever RX is); lanes beside the footprint read zeros.
+//   * A point's taps lie in the pixel range [off, off + L): a warp runs only its steps inside that range.  The step
+//     mask of a point is warp-uniform and lives in uniform registers, so a skipped step costs one uniform branch and
+//     two predicated-off loads, no FMA-pipe time: the rows of the region above and below the footprint are free.
+//   * The tap update of one pixel on one grid is two FFMA2 (fma.rn.f32x2) with the tap as the scalar operand:
+//       acc(re, im) += cre * (vx, vy);   acc(re, im) += cim * (-vy, vx)
+//     (ptxas folds the duplicated tap into the FFMA2's scalar-broadcast operand form), so two 8-byte loads feed
+//     4 * NG FFMA2: the FP32 pipe and the shared-memory port saturate together at NG = 2 and the pipe alone binds at
+//     NG = 4.
+//   * The loads of a point are issued half a point ahead of the FMAs that use them (two halves of the step range, taps
+//     of one half in flight while the other half multiplies), by hand: the branches around the steps keep the
+//     compiler from doing it.
+//   * lra_prepare_kernel first gathers vis / weight in SORTED order and writes, per point, the NG operand pairs
+//     (vx, vy, -vy, vx) = wt*tau*V and the point's slab offset and chunk range as one contiguous record.
+//   * The producer warp walks the batch stream of lra_work.cu and issues, per batch (= up to 12 slab runs of an
+//     item), TMA bulk copies (cp.async.bulk + mbarrier complete_tx): the records of its points and its CF slabs,
+//     from L2 into a ring of shared-memory slots; item boundaries ride in the batch headers, so the consumers
+//     never touch the work list and synchronise once per batch, not once per slab.
+// Regions that fit no (NW, KS) take the global-atomic kernel of lra_grid.cu.
+#pragma once
+#include "lra_region.cuh"
+
+// FMAs of one step: the two pixels of this lane on NG grids, acc[pixel][grid] = (re, im).  `on` is warp-uniform: a
+// real (uniform) branch over the block.
+template <int NG>
+__device__ __forceinline__ void lra_step_fma(lra_u64 (&acc)[2][NG], const lra_u64 (&V)[NG], const lra_u64 (&W)[NG],
+                                             const lra_taps& t, uint32_t on) {
+  if constexpr (NG == 1) {
+    asm volatile(
+        "{\n.reg .pred p;\n.reg .b64 ar, ai, br, bi;\nsetp.eq.u32 p, %8, 0;\n@p bra.uni SKIP_%=;\n"
+        "mov.b64 ar, {%4, %4};\nmov.b64 ai, {%5, %5};\nmov.b64 br, {%6, %6};\nmov.b64 bi, {%7, %7};\n"
+        "fma.rn.f32x2 %0, ar, %2, %0;\nfma.rn.f32x2 %1, br, %2, %1;\n"
+        "fma.rn.f32x2 %0, ai, %3, %0;\nfma.rn.f32x2 %1, bi, %3, %1;\n"
+        "SKIP_%=:\n}"
+        : "+l"(acc[0][0]), "+l"(acc[1][0])
+        : "l"(V[0]), "l"(W[0]), "r"(t.v[0]), "r"(t.v[1]), "r"(t.v[2]), "r"(t.v[3]), "r"(on));
+  }
+  if constexpr (NG == 2) {
+    asm volatile(
+        "{\n.reg .pred p;\n.reg .b64 ar, ai, br, bi;\nsetp.eq.u32 p, %12, 0;\n@p bra.uni SKIP_%=;\n"
+        "mov.b64 ar, {%8, %8};\nmov.b64 ai, {%9, %9};\nmov.b64 br, {%10, %10};\nmov.b64 bi, {%11, %11};\n"
+        "fma.rn.f32x2 %0, ar, %4, %0;\nfma.rn.f32x2 %1, ar, %6, %1;\n"
+        "fma.rn.f32x2 %2, br, %4, %2;\nfma.rn.f32x2 %3, br, %6, %3;\n"
+        "fma.rn.f32x2 %0, ai, %5, %0;\nfma.rn.f32x2 %1, ai, %7, %1;\n"
+        "fma.rn.f32x2 %2, bi, %5, %2;\nfma.rn.f32x2 %3, bi, %7, %3;\n"
+        "SKIP_%=:\n}"
+        : "+l"(acc[0][0]), "+l"(acc[0][1]), "+l"(acc[1][0]), "+l"(acc[1][1])
+        : "l"(V[0]), "l"(W[0]), "l"(V[1]), "l"(W[1]), "r"(t.v[0]), "r"(t.v[1]), "r"(t.v[2]), "r"(t.v[3]), "r"(on));
+  }
+  if constexpr (NG == 3) {
+    asm volatile(
+        "{\n.reg .pred p;\n.reg .b64 ar, ai, br, bi;\nsetp.eq.u32 p, %16, 0;\n@p bra.uni SKIP_%=;\n"
+        "mov.b64 ar, {%12, %12};\nmov.b64 ai, {%13, %13};\nmov.b64 br, {%14, %14};\nmov.b64 bi, {%15, %15};\n"
+        "fma.rn.f32x2 %0, ar, %6, %0;\nfma.rn.f32x2 %1, ar, %8, %1;\n"
+        "fma.rn.f32x2 %2, ar, %10, %2;\nfma.rn.f32x2 %3, br, %6, %3;\n"
+        "fma.rn.f32x2 %4, br, %8, %4;\nfma.rn.f32x2 %5, br, %10, %5;\n"
+        "fma.rn.f32x2 %0, ai, %7, %0;\nfma.rn.f32x2 %1, ai, %9, %1;\n"
+        "fma.rn.f32x2 %2, ai, %11, %2;\nfma.rn.f32x2 %3, bi, %7, %3;\n"
+        "fma.rn.f32x2 %4, bi, %9, %4;\nfma.rn.f32x2 %5, bi, %11, %5;\n"
+        "SKIP_%=:\n}"
+        : "+l"(acc[0][0]), "+l"(acc[0][1]), "+l"(acc[0][2]), "+l"(acc[1][0]), "+l"(acc[1][1]), "+l"(acc[1][2])
+        : "l"(V[0]), "l"(W[0]), "l"(V[1]), "l"(W[1]), "l"(V[2]), "l"(W[2]), "r"(t.v[0]), "r"(t.v[1]), "r"(t.v[2]), "r"(t.v[3]), "r"(on));
+  }
+  if constexpr (NG == 4) {
+    asm volatile(
+        "{\n.reg .pred p;\n.reg .b64 ar, ai, br, bi;\nsetp.eq.u32 p, %20, 0;\n@p bra.uni SKIP_%=;\n"
+        "mov.b64 ar, {%16, %16};\nmov.b64 ai, {%17, %17};\nmov.b64 br, {%18, %18};\nmov.b64 bi, {%19, %19};\n"
+        "fma.rn.f32x2 %0, ar, %8, %0;\nfma.rn.f32x2 %1, ar, %10, %1;\n"
+        "fma.rn.f32x2 %2, ar, %12, %2;\nfma.rn.f32x2 %3, ar, %14, %3;\n"
+        "fma.rn.f32x2 %4, br, %8, %4;\nfma.rn.f32x2 %5, br, %10, %5;\n"
+        "fma.rn.f32x2 %6, br, %12, %6;\nfma.rn.f32x2 %7, br, %14, %7;\n"
+        "fma.rn.f32x2 %0, ai, %9, %0;\nfma.rn.f32x2 %1, ai, %11, %1;\n"
+        "fma.rn.f32x2 %2, ai, %13, %2;\nfma.rn.f32x2 %3, ai, %15, %3;\n"
+        "fma.rn.f32x2 %4, bi, %9, %4;\nfma.rn.f32x2 %5, bi, %11, %5;\n"
+        "fma.rn.f32x2 %6, bi, %13, %6;\nfma.rn.f32x2 %7, bi, %15, %7;\n"
+        "SKIP_%=:\n}"
+        : "+l"(acc[0][0]), "+l"(acc[0][1]), "+l"(acc[0][2]), "+l"(acc[0][3]), "+l"(acc[1][0]), "+l"(acc[1][1]), "+l"(acc[1][2]), "+l"(acc[1][3])
+        : "l"(V[0]), "l"(W[0]), "l"(V[1]), "l"(W[1]), "l"(V[2]), "l"(W[2]), "l"(V[3]), "l"(W[3]), "r"(t.v[0]), "r"(t.v[1]), "r"(t.v[2]), "r"(t.v[3]), "r"(on));
+  }
+}
+
+// Steps [B, E) of a point, unrolled: loads and FMAs.
+template <int NW, int NG, int KS, int B, int E>
+struct lra_steps {
+  static __device__ __forceinline__ void load(lra_taps (&T)[KS], uint32_t addr, uint32_t mask) {
+    if constexpr (B < E) {
+      lra_step_load<B * 512 * NW>(T[B], addr, mask & (1u << B));
+      lra_steps<NW, NG, KS, B + 1, E>::load(T, addr, mask);
+    }
+  }
+  static __device__ __forceinline__ void fma(lra_u64 (&acc)[KS][2][NG], const lra_u64 (&V)[NG], const lra_u64 (&W)[NG],
+                                             const lra_taps (&T)[KS], uint32_t mask) {
+    if constexpr (B < E) {
+      lra_step_fma<NG>(acc[B], V, W, T[B], mask & (1u << B));
+      lra_steps<NW, NG, KS, B + 1, E>::fma(acc, V, W, T, mask);
+    }
+  }
+};
+
+// One point as a consumer warp sees it: operand pairs per grid, address of the lane's first tap, step mask.
+template <int NG>
+struct lra_point {
+  lra_u64 V[NG], W[NG];   // (vx, vy), (-vy, vx)
+  uint32_t addr, mask;
+};
+// rec: the point's record in the slot (lra_point_bytes); lane_base: shared-memory address of the slot's slab area
+// + 8 * (64 * warp + lane).  mask bit s is set iff chunk NW*s + warp lies in the point's chunk range [c_lo, c_hi].
+template <int NW, int NG>
+__device__ __forceinline__ lra_point<NG> lra_get_point(const unsigned char* rec, uint32_t lane_base, int warp, bool valid) {
+  lra_point<NG> p;
+#pragma unroll
+  for (int g = 0; g < NG; ++g) {
+    const ulonglong2 v = *reinterpret_cast<const ulonglong2*>(rec + 16 * g);
+    p.V[g] = v.x; p.W[g] = v.y;
+  }
+  const uint2 wc = *reinterpret_cast<const uint2*>(rec + 16 * NG);
+  p.mask = valid ? lra_step_mask<NW>(wc.y, warp) : 0u;
+  p.addr = lane_base + wc.x;
+  return p;
+}
+
+template <int NW, int KS, int NG>
+__global__ void __launch_bounds__((NW + 1) * 32) __maxnreg__(LRA_MAXNREG(NW, KS, NG, false)) lra_grid_region_kernel(const lra_region_args a) {
+  extern __shared__ __align__(128) unsigned char smem[];
+  const int lane = threadIdx.x & 31;
+  const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);   // provably warp-uniform: uniform registers
+  const uint32_t sbase = lra_smem_u32(smem);
+  const uint32_t full0 = sbase, empty0 = sbase + 128, slots0 = sbase + LRA_RING_HDR;
+  lra_region_ring_init<NW>(a, smem, full0, empty0);
+  constexpr int PB = lra_point_bytes(NG);
+  if (warp == NW) {
+    lra_region_producer<NW, 0>(a, a.prep, PB, smem + LRA_RING_HDR, full0, empty0, slots0);
+    return;
+  }
+  // -------------------------------------------------------------------- consumer warps
+  constexpr int KA = (KS + 1) / 2;   // steps [0, KA): first half, [KA, KS): second half
+  lra_u64 acc[KS][2][NG];
+#pragma unroll
+  for (int s = 0; s < KS; ++s)
+#pragma unroll
+    for (int g = 0; g < NG; ++g) acc[s][0][g] = acc[s][1][g] = 0ull;
+  lra_taps T[KS];
+#pragma unroll
+  for (int s = 0; s < KS; ++s) T[s].v[0] = T[s].v[1] = T[s].v[2] = T[s].v[3] = 0u;
+  uint32_t slot = 0, par = 0;
+  const uint32_t lane_off = (uint32_t)a.slab0 + 8u * (64u * warp + lane);
+  for (;;) {
+    lra_mbar_wait(full0 + 8 * slot, par);
+    const unsigned char* sp = smem + LRA_RING_HDR + (size_t)slot * a.slot_bytes;
+    const uint4 h = *reinterpret_cast<const uint4*>(sp);
+    const unsigned count = h.y & 0xff;
+    const uint32_t lane_base = slots0 + slot * a.slot_bytes + lane_off;
+    const unsigned char* rec = sp + LRA_SLOT_VAL;
+    // software pipeline over the points of the batch: the loads of a half are in flight while the other half multiplies
+    lra_point<NG> cur = lra_get_point<NW, NG>(rec, lane_base, warp, count > 0);
+    lra_steps<NW, NG, KS, 0, KA>::load(T, cur.addr, cur.mask);
+    for (unsigned q = 0; q < count; ++q) {
+      rec += PB;
+      const lra_point<NG> nxt = lra_get_point<NW, NG>(rec, lane_base, warp, q + 1 < count);
+      lra_steps<NW, NG, KS, KA, KS>::load(T, cur.addr, cur.mask);
+      lra_steps<NW, NG, KS, 0, KA>::fma(acc, cur.V, cur.W, T, cur.mask);
+      lra_steps<NW, NG, KS, 0, KA>::load(T, nxt.addr, nxt.mask);
+      lra_steps<NW, NG, KS, KA, KS>::fma(acc, cur.V, cur.W, T, cur.mask);
+      cur = nxt;
+    }
+    __syncwarp();
+    if (lane == 0) lra_mbar_arrive(empty0 + 8 * slot);
+    if (h.y & LRA_BATCH_LAST) {
+      // ---- row a4: add the item's region to the grid, once ----
+      const int hh = (a.S - 1) >> 1;
+      const int ty = (int)(h.w / (unsigned)a.ntx), tx = (int)(h.w - (unsigned)ty * a.ntx);
+      const int x0 = tx * a.tile_x - hh, y0 = ty * a.tile_y - hh;
+      const unsigned magic = 0xffffffffu / (unsigned)a.rx + 1u;
+#pragma unroll
+      for (int s = 0; s < KS; ++s) {
+#pragma unroll
+        for (int half = 0; half < 2; ++half) {
+          const unsigned e = 64u * (NW * s + warp) + 32u * half + lane;
+          const int y = (int)__umulhi(e, magic), x = (int)e - y * a.rx;
+          const int gx = x0 + x, gy = y0 + y;
+          const bool ok = y < a.ry && gx >= 0 && gx < a.nx && gy >= 0 && gy < a.ny;
+#pragma unroll
+          for (int g = 0; g < NG; ++g) {
+            float vr, vi;
+            lra_unpack2(acc[s][half][g], vr, vi);
+            if (ok && (vr != 0.f || vi != 0.f)) lra_red_add_v2(a.grid + (size_t)g * a.plane + (size_t)gy * a.nx + gx, vr, vi);
+            acc[s][half][g] = 0ull;
+          }
+        }
+      }
+    }
+    if (h.y & LRA_BATCH_END) break;
+    if (++slot == (uint32_t)a.nslot) { slot = 0; par ^= 1; }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
+template <int NW, int KS, int NG>
+static int lra_grid_launch_class(lra_plan* p, lra_region_args a, const lra_geom& q, int c, cudaStream_t st) {
+  int smem = 0;
+  if (!lra_region_ring(q, lra_grids_per_pass(p->ncorr * p->nterms), false, lra_point_bytes(NG), &a, &smem)) return LRA_EINVAL;
+  auto kern = lra_grid_region_kernel<NW, KS, NG>;
+  static int attr_smem[LRA_MAX_DEVICES];   // per instantiation and device: the opt-in is made once, not per launch
+  if (p->device < 0 || p->device >= LRA_MAX_DEVICES || attr_smem[p->device] < smem) {
+    LRA_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    if (p->device >= 0 && p->device < LRA_MAX_DEVICES) attr_smem[p->device] = smem;
+  }
+  a.work = p->work + p->item_off[c];
+  a.n_items = (unsigned)p->n_items[c];
+  a.batch = reinterpret_cast<const uint4*>(p->batch) + (size_t)p->batch_off[c] * 4;
+  int ctas = p->sm_count * lra_ctas_per_sm(NW, KS, lra_grids_per_pass(p->ncorr * p->nterms), false);   // what the ring was sized for
+  if ((int64_t)ctas > p->n_items[c]) ctas = (int)p->n_items[c];
+  kern<<<ctas, (NW + 1) * 32, smem, st>>>(a);
+  LRA_LAUNCH_CHECK(p);
+  return LRA_OK;
+}
+
+template <int NW, int NG>
+static int lra_grid_launch_ks(lra_plan* p, const lra_region_args& a, const lra_geom& q, int c, cudaStream_t st) {
+  // the (NW, KS) of a class come from the plan's grids per pass; a remainder pass of fewer grids runs the same steps
+  switch (q.ks) {
+    case 1: return lra_grid_launch_class<NW, 1, NG>(p, a, q, c, st);
+    case 2: return lra_grid_launch_class<NW, 2, NG>(p, a, q, c, st);
+    case 3: return lra_grid_launch_class<NW, 3, NG>(p, a, q, c, st);
+    case 4: return lra_grid_launch_class<NW, 4, NG>(p, a, q, c, st);
+    default: break;
+  }
+  if constexpr (NG <= 2) {
+    if (q.ks == 6) return lra_grid_launch_class<NW, 6, NG>(p, a, q, c, st);
+  }
+  if constexpr (NG == 1) {
+    if (q.ks == 8) return lra_grid_launch_class<NW, 8, NG>(p, a, q, c, st);
+  }
+  return LRA_EINVAL;
+}
+
+// One launch: the items of support class c, NG grids starting at a.grid.
+template <int NG>
+int lra_grid_launch_ng(lra_plan* p, const lra_region_args& a, const lra_geom& q, int c, cudaStream_t st) {
+  switch (q.nw) {
+    case 1: return lra_grid_launch_ks<1, NG>(p, a, q, c, st);
+    case 2: return lra_grid_launch_ks<2, NG>(p, a, q, c, st);
+    case 4: return lra_grid_launch_ks<4, NG>(p, a, q, c, st);
+    case 8: return lra_grid_launch_ks<8, NG>(p, a, q, c, st);
+    case 16: return lra_grid_launch_ks<16, NG>(p, a, q, c, st);
+    default: return LRA_EINVAL;
+  }
+}

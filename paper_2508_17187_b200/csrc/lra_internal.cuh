@@ -15,7 +15,6 @@
 //   w: S | cf << 8          (support in pixels, kernel number)
 typedef uint4 lra_rec;
 
-#define LRA_NGROUP 5   // kernel configurations of the region gridder / degridder; the last one is the fallback
 #define LRA_NCLASS 65  // support classes: class (S - 1) / 2 for S = 1, 3, .., 129
 #define LRA_NAUX 4     // internal streams the per-class launches of one call are spread over
 #define LRA_MAX_DEVICES 64
@@ -28,11 +27,11 @@ struct lra_plan {
   cudaStream_t stream;
   std::vector<int32_t> cf_support;
   std::vector<int64_t> slab_off;   // float offset of slab (cf, 0, 0) in `slabs`
-  std::vector<int32_t> slab_stride;  // floats per slab of kernel cf: 2 * lra_plane_floats(S, tile_x)
+  std::vector<int32_t> slab_stride;  // floats per slab of kernel cf: 2 * lra_slab_complex(S, tile_x)
   int32_t max_support;
   int32_t ntx, nty, ntiles;
   // ---- device: CF store ----
-  float* slabs;             // [cf][fy][fx] phase-major PLANAR slabs, see lra_plane_floats()
+  float* slabs;             // [cf][fy][fx] phase-major slabs of interleaved complex taps, see lra_slab_complex()
   int64_t slab_elems;       // total floats
   int32_t* d_cf_support;    // [n_cf]
   int64_t* d_slab_off;      // [n_cf]
@@ -80,12 +79,12 @@ struct lra_plan {
 // Slab layout (one slab = the S*S taps of one kernel at one sub-pixel phase, what one visibility point needs).
 // A region kernel works on a REGION of RX = S + tile_x - 1 columns (tile + halo) whose pixels are numbered
 // e = y*RX + x, and it reads the tap that a point with footprint origin (ox, oy) puts on pixel e at the linear
-// slab index e - (oy*RX + ox).  So a slab is stored with the region's pitch: two planes (real parts, then
-// imaginary parts) of PF = lra_plane_floats(S, tile_x) floats, tap (j, i), 0 <= j, i < S, at float j*RX + i, and the
-// RX - S pad floats that end each row ZERO.  A lane that looks at a pixel beside the footprint therefore reads a
-// zero instead of branching (the zeros above and below the footprint live in shared memory, lra_pipe.cuh).
-// PF is a multiple of 4 (16 bytes) so that one TMA bulk copy moves a plane.
-__host__ __device__ inline int lra_plane_floats(int S, int tile_x) { return (S * (S + tile_x - 1) + 3) & ~3; }
+// slab index e - (oy*RX + ox).  So a slab is stored with the region's pitch, as interleaved COMPLEX values (one
+// 8-byte shared-memory load gives a lane its tap): tap (j, i), 0 <= j, i < S, at complex index j*RX + i, and the
+// RX - S pad values that end each row ZERO.  A lane that looks at a pixel beside the footprint therefore reads a
+// zero instead of branching (the zeros before and after the slab live in shared memory, lra_pipe.cuh).
+// The slab is rounded up to an even number of complex values (16 bytes) so that one TMA bulk copy moves it.
+__host__ __device__ inline int lra_slab_complex(int S, int tile_x) { return (S * (S + tile_x - 1) + 1) & ~1; }
 __host__ __device__ inline int lra_tap_index(int S, int tile_x, int j, int i) { return j * (S + tile_x - 1) + i; }
 
 #define LRA_CUDA(p, call)                         \

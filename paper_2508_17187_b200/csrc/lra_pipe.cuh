@@ -14,61 +14,92 @@
 #define LRA_SLOTS_TARGET 2   // ring slots per CTA the batch size is chosen for
 #endif
 #ifndef LRA_CTA_CAP
-#define LRA_CTA_CAP 10      // CTAs per SM at most
+#define LRA_CTA_CAP 12      // CTAs per SM at most
 #endif
-#ifndef LRA_REGS_PER_STEP
-#define LRA_REGS_PER_STEP 12   // 8 accumulators + 4 taps in flight per step; 10 (one more CTA per SM) measured no faster
-#endif
-#define LRA_KSMAX 9        // steps per consumer warp at most: 9 * 2 pixels * 2 grids * (re, im) = 72 accumulators
+#define LRA_KSCAP 8         // steps per consumer warp at most (the step mask of a point is 8 bits wide)
+#define LRA_NGMAX 4         // grids per pass at most (more grids: several passes over the same batch stream)
+#define LRA_GAP 64          // complex zeros before, between and after the slabs of a ring slot
 
 typedef unsigned long long lra_u64;
 
 // ---------------------------------------------------------------------------------------------------
 // Geometry of a support class.  A region kernel keeps a region of RX*RY pixels (tile + halo, RX = tile_x + S - 1,
-// RY = tile + S - 1) in the registers of NW consumer warps: pixel e = y*RX + x belongs to warp (e / 64) % NW, step
-// e / (64*NW), lane e % 32, half (e / 32) % 2, i.e. at step s a warp owns the 64 consecutive pixels that start at
-// 64*(NW*s + warp) and a lane owns two of them, 32 apart (the two halves of one FFMA2).  NW = 2, 4, 8 or 16 is the
-// smallest for which ks = ceil(RX*RY / (64*NW)) <= lra_ks_max(NW) (the register budget that still leaves two CTAs of
-// NW = 8 on an SM); a region too large for NW = 16 goes to the fallback kernels (global atomics).  Every lane reads a
-// tap for every point, at linear slab index e - off with
-// off = oy*RX + ox <= pre, so a slab plane sits in shared memory between zeros: `gap` floats before (>= pre) and
-// after (>= the pixels past the last tap) -- consecutive planes share a gap, which no copy ever writes.
+// RY = tile + S - 1) in the registers of NW consumer warps: pixel e = y*RX + x belongs to chunk e / 64; chunk c
+// belongs to warp c % NW, step c / NW, i.e. at step s a warp owns the 64 consecutive pixels that start at
+// 64*(NW*s + warp) and a lane owns two of them, 32 apart, each as one complex accumulator (an aligned register
+// pair) per grid.  NW = 1, 2, 4, 8 or 16 is the smallest for which KS = ceil(chunks / NW) <= lra_ks_max(grids per
+// pass); KS is rounded up to an even number where that still fits (fewer kernel instantiations; the surplus steps are
+// never active).  A region too large for NW = 16 goes to the fallback kernels (global atomics).
+// A point with footprint origin (ox, oy) inside the region puts tap (j, i) on pixel off + j*RX + i, off = oy*RX + ox,
+// so its taps lie in the pixel range [off, off + L), L = (S-1)*RX + S: a lane reads the tap of pixel e at linear slab
+// index e - off, and only the chunks c_lo = off/64 .. c_hi = (off + L - 1)/64 of the region are visited (the rest of
+// the region lies above or below the footprint).  Inside the visited range a lane beside the footprint reads one
+// of the zeros that end every slab row, or one of the LRA_GAP zeros around the slab in shared memory.
 // ---------------------------------------------------------------------------------------------------
 struct lra_geom {
-  int S, rx, ry, group, nw, ks;   // group = log2(nw) - 1, or LRA_NGROUP - 1 for the fallback
-  int core;                       // floats per slab plane as stored and copied (lra_plane_floats)
-  int gap, stride;                // floats of zeros between planes; stride = core + gap
+  int S, rx, ry, nw, ks;          // nw = 0: the fallback kernels
+  int span;                       // L: pixels from the first to the last tap of a footprint
+  int core;                       // complex values per slab as stored and copied (lra_slab_complex)
+  int stride;                     // core + LRA_GAP
   int per_batch;                  // slab runs per batch
 };
-#ifndef LRA_KSLIM
-#define LRA_KSLIM 9
-#endif
-__host__ __device__ constexpr int lra_ks_max(int nw) { return nw == 16 ? LRA_KSMAX : nw == 8 ? (LRA_KSLIM < 7 ? LRA_KSLIM : 7) : LRA_KSLIM; }
-// CTAs per SM the (NW, KS) kernel is built for: ~12 registers per step (8 accumulators, 4 taps in flight) + 36.
-__host__ __device__ constexpr int lra_ctas_per_sm(int nw, int ks) {
-  if (nw == 8 && ks == 7) return 2;   // 112 registers: measured without spills
-  const int regs = (LRA_REGS_PER_STEP * ks + 36 + 7) / 8 * 8, r = 65536 / ((nw + 1) * 32 * regs);
-  return r < 1 ? 1 : r > LRA_CTA_CAP ? LRA_CTA_CAP : r;
+__host__ __device__ constexpr int lra_ks_max(int ngp) { return ngp == 1 ? 8 : ngp == 2 ? 6 : 4; }
+__host__ __device__ constexpr int lra_grids_per_pass(int ng) { return ng < LRA_NGMAX ? ng : LRA_NGMAX; }
+// Registers per thread the (NW, KS, NG) kernels are built for.  lra_regs_need: the fewest registers (a multiple of 8)
+// with which ptxas builds the kernel without spilling (per step 4 accumulators per grid and 4 tap values in flight,
+// plus addressing and the point's values; the degridder also holds the partial sums of four points), found by
+// compiling every (KS, NG) under a range of register limits.  CTAs per SM follow from it, and the kernel is then given
+// all the registers that this number of CTAs leaves (lra_regs).
+__host__ __device__ constexpr int lra_regs_need(int ks, int ngp, bool degrid) {
+  // rows: grids per pass 1..4; columns: KS 1..8
+  constexpr int G[4][8] = {{48, 48, 56, 64, 80, 80, 104, 104}, {48, 56, 64, 80, 120, 120, 120, 120}, {64, 72, 88, 112, 112, 112, 112, 112}, {80, 96, 120, 136, 136, 136, 136, 136}};
+  constexpr int D[4][8] = {{48, 56, 56, 64, 80, 80, 96, 96}, {56, 64, 64, 80, 112, 112, 112, 112}, {64, 80, 96, 112, 112, 112, 112, 112}, {72, 104, 120, 136, 136, 136, 136, 136}};
+  return degrid ? D[ngp - 1][ks - 1] : G[ngp - 1][ks - 1];
 }
-// Shared memory of a CTA and of one ring slot (3 slots per CTA at least, whenever a slab fits).
-__host__ __device__ constexpr int lra_cta_smem(int nw, int ks) { return (227 * 1024) / lra_ctas_per_sm(nw, ks) - 1024; }
-__host__ __device__ inline lra_geom lra_make_geom(int S, int tile_x, int tile_y) {
+// The register file is 16384 registers per SM sub-partition and the warps of the resident CTAs are dealt round to the
+// four sub-partitions: C CTAs of NW + 1 warps put ceil((NW + 1) * C / 4) warps on the fullest one.
+__host__ __device__ constexpr int lra_warps_per_smsp(int nw, int ctas) { return ((nw + 1) * ctas + 3) / 4; }
+__host__ __device__ constexpr int lra_ctas_per_sm(int nw, int ks, int ngp, bool degrid) {
+  int r = 1;
+  while (r < LRA_CTA_CAP && (nw + 1) * (r + 1) <= 64 && lra_warps_per_smsp(nw, r + 1) * 32 * lra_regs_need(ks, ngp, degrid) <= 16384) ++r;
+  return r;
+}
+__host__ __device__ constexpr int lra_regs(int nw, int ks, int ngp, bool degrid) {
+  const int r = 16384 / (32 * lra_warps_per_smsp(nw, lra_ctas_per_sm(nw, ks, ngp, degrid))) / 8 * 8;
+  return r > 168 ? 168 : r;
+}
+#ifdef LRA_FORCE_NREG   // build aid: find the registers a kernel needs
+#define LRA_MAXNREG(nw, ks, ng, degrid) (LRA_FORCE_NREG + 0 * (ks))
+#else
+#define LRA_MAXNREG(nw, ks, ng, degrid) lra_regs(nw, ks, ng, degrid)
+#endif
+// Shared memory of a CTA.  The batch stream (lra_work.cu) is cut for the gridder's CTAs, the smaller ones.
+__host__ __device__ constexpr int lra_cta_smem(int nw, int ks, int ngp, bool degrid) { return (227 * 1024) / lra_ctas_per_sm(nw, ks, ngp, degrid) - 1024; }
+// Bytes per point in a ring slot: gridder 16 per grid (vx, vy, -vy, vx) + 16 (word, chunk range); degridder 16 (the
+// pw record) + 8 per grid (results).
+__host__ __device__ constexpr int lra_point_bytes(int ngp) { return 16 * ngp + 16; }
+__host__ __device__ inline lra_geom lra_make_geom(int S, int tile_x, int tile_y, int ng) {
   lra_geom q;
+  const int ngp = lra_grids_per_pass(ng);
   q.S = S; q.rx = S + tile_x - 1; q.ry = S + tile_y - 1;
-  const int slots = q.rx * q.ry;
-  q.group = LRA_NGROUP - 1; q.nw = 0; q.ks = 0;
-  for (int g = 0; g < LRA_NGROUP - 1; ++g)
-    if (slots <= 64 * (2 << g) * lra_ks_max(2 << g)) { q.group = g; q.nw = 2 << g; q.ks = (slots + 64 * q.nw - 1) / (64 * q.nw); break; }
-  q.core = lra_plane_floats(S, tile_x);
-  const int pre = (tile_y - 1) * q.rx + tile_x - 1, post = 64 * q.nw * q.ks - S * q.rx;
-  q.gap = ((pre > post ? pre : post) + 3) & ~3;
-  q.stride = q.core + q.gap;
+  q.span = (S - 1) * q.rx + S;
+  const int chunks = (q.rx * q.ry + 63) / 64;
+  q.nw = 0; q.ks = 0;
+  for (int nw = 1; nw <= 16; nw <<= 1) {
+    int ks = (chunks + nw - 1) / nw;
+    if (ks > lra_ks_max(ngp)) continue;
+    if ((ks & 1) && ks + 1 <= lra_ks_max(ngp) && ngp < 4) ++ks;
+    q.nw = nw; q.ks = ks;
+    break;
+  }
+  q.core = lra_slab_complex(S, tile_x);
+  q.stride = q.core + LRA_GAP;
   q.per_batch = 1;
-  if (q.group < LRA_NGROUP - 1) {   // a third of the CTA's shared memory per slot: 384 bytes of values + a slab per run
-    const int r = ((lra_cta_smem(q.nw, q.ks) - 512) / LRA_SLOTS_TARGET - 256 - 4 * q.gap) / (LRA_RUNMAX * 64 + 8 * q.stride);
+  if (q.nw) {
+    const int r = ((lra_cta_smem(q.nw, q.ks, ngp, false) - 512) / LRA_SLOTS_TARGET - 256 - 8 * LRA_GAP) / (LRA_RUNMAX * lra_point_bytes(ngp) + 8 * q.stride);
     q.per_batch = r < 1 ? 1 : r > LRA_BATCH_SLABS ? LRA_BATCH_SLABS : r;
-    // even one slab per slot must fit the CTA's shared memory (values + record + ring header: 1 KB), else fall back
-    if (4 * (q.gap + 2 * q.stride) + 1024 > lra_cta_smem(q.nw, q.ks)) { q.group = LRA_NGROUP - 1; q.per_batch = 1; }
+    // even one slab per slot must fit the CTA's shared memory (values + record + ring header: 1.5 KB), else fall back
+    if (8 * (LRA_GAP + q.stride) + LRA_RUNMAX * lra_point_bytes(ngp) + 1536 > lra_cta_smem(q.nw, q.ks, ngp, false)) { q.nw = 0; q.ks = 0; q.per_batch = 1; }
   }
   return q;
 }
@@ -83,9 +114,10 @@ __host__ __device__ inline int lra_class_of(int S) { return (S - 1) >> 1; }
 //   batch = per_batch consecutive runs of one item: what occupies one slot of a CTA's shared-memory ring.
 //           64 bytes: uint4 {first sorted position, count | flags, runs, tile id}, then the slab offsets of its
 //           runs in 16-byte units (uint32 x 12).  LRA_BATCH_LAST marks the last batch of its item.
-//   pw    = for every sorted position 16 bytes (one TMA granule) {word, k, S, 0}; word = the byte offset, inside the
-//           slot's slab area, of the float the lane that owns pixel 0 of the region reads for this point:
-//           4 * (gap + run * 2 * stride - (oy*RX + ox)).
+//   pw    = for every sorted position 16 bytes (one TMA granule) {word, k, S, c_lo | c_hi << 16}; word = the byte
+//           offset (signed), inside the slot's slab area, of the complex value the lane that owns pixel 0 of the
+//           region would read for this point: 8 * (LRA_GAP + run * stride - off), off = oy*RX + ox; c_lo, c_hi =
+//           first and last chunk of the region that the footprint touches.
 // ---------------------------------------------------------------------------------------------------
 #define LRA_BATCH_LAST 0x40000000u
 #define LRA_BATCH_END 0x80000000u

@@ -13,32 +13,26 @@ struct lra_nvtx_range {
   ~lra_nvtx_range() { nvtxRangePop(); }
 };
 
-// Re-lay one oversampled kernel into phase-major planar slabs (reading R3; layout in
-// lra_internal.cuh):  tap (j + h, i + h) of slab (fyi, fxi) = K[(j*os - fy) + c0][(i*os - fx) + c0],
+// Re-lay one oversampled kernel into phase-major slabs of interleaved complex taps (reading
+// R3; layout in lra_internal.cuh):  tap (j + h, i + h) of slab (fyi, fxi) = K[(j*os - fy) + c0][(i*os - fx) + c0],
 //   fy = fyi - os/2, c0 = h*os + (os-1-os/2).
-// One thread per output float; the padding floats are zero-filled.
-__global__ void lra_relayout_kernel(const float2* __restrict__ K, float* __restrict__ slab, int S, int os,
-                                    int slab_stride, int tile_x) {
+// One thread per output complex value; the padding values are zero-filled.
+__global__ void lra_relayout_kernel(const float2* __restrict__ K, float2* __restrict__ slab, int S, int os,
+                                    int slab_complex, int tile_x) {
   const int h = (S - 1) / 2;
   const int rx = S + tile_x - 1;
   const int c0 = h * os + (os - 1 - os / 2);
-  const int pf = slab_stride >> 1;
-  const int64_t n = (int64_t)os * os * slab_stride;
+  const int64_t n = (int64_t)os * os * slab_complex;
   const int64_t ld = (int64_t)S * os;
   for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
-    int phase = (int)(e / slab_stride), t = (int)(e % slab_stride);
-    const int im = t >= pf;
-    if (im) t -= pf;
-    float v = 0.f;
-    {
-      int jj = t / rx, ii = t - jj * rx;
-      if (jj < S && ii < S) {
-        int fyi = phase / os, fxi = phase % os;
-        int j = jj - h, i = ii - h;
-        int row = j * os - (fyi - os / 2) + c0, col = i * os - (fxi - os / 2) + c0;
-        float2 k = K[row * ld + col];
-        v = im ? k.y : k.x;
-      }
+    const int phase = (int)(e / slab_complex), t = (int)(e % slab_complex);
+    float2 v = make_float2(0.f, 0.f);
+    const int jj = t / rx, ii = t - jj * rx;
+    if (jj < S && ii < S) {
+      const int fyi = phase / os, fxi = phase % os;
+      const int j = jj - h, i = ii - h;
+      const int row = j * os - (fyi - os / 2) + c0, col = i * os - (fxi - os / 2) + c0;
+      v = K[row * ld + col];
     }
     slab[e] = v;
   }
@@ -79,7 +73,7 @@ extern "C" int lra_plan_create(lra_plan** out, const lra_plan_desc* d) {
   p->max_support = 1;
   for (int c = 0; c < d->n_cf; ++c) {
     int S = p->cf_support[c];
-    p->slab_stride[c] = 2 * lra_plane_floats(S, tile_x);
+    p->slab_stride[c] = 2 * lra_slab_complex(S, tile_x);
     p->slab_off[c] = total;
     total += (int64_t)p->os * p->os * p->slab_stride[c];
     int64_t n_in = (int64_t)S * p->os * S * p->os;
@@ -116,10 +110,11 @@ extern "C" int lra_plan_create(lra_plan** out, const lra_plan_desc* d) {
     int64_t n_in = (int64_t)S * p->os * S * p->os;
     const float2* src = (const float2*)d->cf_data + d->cf_offset[c];
     CK(cudaMemcpyAsync(staging, src, (size_t)n_in * sizeof(float2), cudaMemcpyHostToDevice, p->stream));
-    int64_t n_out = (int64_t)p->os * p->os * p->slab_stride[c];
+    int64_t n_out = (int64_t)p->os * p->os * (p->slab_stride[c] / 2);
     int blocks = (int)((n_out + 255) / 256);
     if (blocks > 4096) blocks = 4096;
-    lra_relayout_kernel<<<blocks, 256, 0, p->stream>>>(staging, p->slabs + p->slab_off[c], S, p->os, p->slab_stride[c], tile_x);
+    lra_relayout_kernel<<<blocks, 256, 0, p->stream>>>(staging, reinterpret_cast<float2*>(p->slabs + p->slab_off[c]), S, p->os,
+                                                       p->slab_stride[c] / 2, tile_x);
     p->launches++;
     CK(cudaGetLastError());
   }

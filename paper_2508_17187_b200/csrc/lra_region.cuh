@@ -10,20 +10,20 @@ struct lra_region_args {
   unsigned long long* ticket;
   const uint4* batch;           // batch records of this class (4 x uint4 each)
   const float* slabs;
-  const float* prep;            // this pass: [sorted position][NG][8]
+  const void* prep;             // this pass: per sorted position lra_point_bytes (gridder) or the 16-byte pw record
   float2* grid;                 // first grid of this pass
   long long plane;              // pixels per grid
   int nx, ny, tile_x, tile_y, ntx;
   int S, rx, ry, ks;            // the class's geometry (lra_make_geom)
-  int core_bytes, stride_bytes, gap_bytes;   // slab plane as copied; plane + zeros; zeros before the first plane
+  int core_bytes, stride_bytes, gap_bytes;   // slab as copied; slab + zeros; zeros before the first slab
   int nslot, slot_bytes, slab0; // ring geometry: slots, bytes per slot, offset of the slab area inside a slot
   int out_off;                  // degridder: offset of the per-point results inside a slot
   float2* res;                  // degridder: this pass's results, [sorted position][grids of the pass]
 };
 
-// slot layout (bytes): batch record (64) | pad | prepared values | slab area.  The slab area is gap, re plane of run
-// 0, gap, im plane of run 0, gap, re plane of run 1, ...: the kernel zeroes it once and the copies only ever write
-// the planes, so the gaps stay zero for the whole launch (one launch = one support class = one geometry).
+// slot layout (bytes): batch record (64) | pad | per-point values | slab area.  The slab area is gap, slab of run 0,
+// gap, slab of run 1, ...: the kernel zeroes it once and the copies only ever write the slabs, so the gaps stay
+// zero for the whole launch (one launch = one support class = one geometry).
 #define LRA_SLOT_VAL 128
 #define LRA_RING_HDR 256   // full / empty barriers of up to 16 slots
 
@@ -84,7 +84,7 @@ __device__ __forceinline__ void lra_region_producer(const lra_region_args& a, co
           const bool pv = vals != nullptr;
           lra_mbar_wait(empty0 + 8 * slot, par ^ 1);
           asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(sa), "r"(cur.x), "r"(cur.y), "r"(cur.z), "r"(cur.w) : "memory");
-          lra_mbar_arrive_expect_tx(fb, (pv ? count * val_bytes : 0u) + nr * 2u * (uint32_t)a.core_bytes);
+          lra_mbar_arrive_expect_tx(fb, (pv ? count * val_bytes : 0u) + nr * (uint32_t)a.core_bytes);
           if (pv) lra_tma_load_1d(sa + LRA_SLOT_VAL, reinterpret_cast<const unsigned char*>(vals) + (size_t)cur.x * val_bytes, count * val_bytes, fb);
         }
         __syncwarp();   // the slot is free from here on
@@ -96,9 +96,7 @@ __device__ __forceinline__ void lra_region_producer(const lra_region_args& a, co
           const uint32_t off16 = __shfl_sync(0xffffffffu, pick, 4 * j + 1 + (r >> 2));
           if (lane == 0) {
             const unsigned char* src_b = reinterpret_cast<const unsigned char*>(a.slabs) + ((size_t)off16 << 4);
-            const uint32_t dst = sa + slab0 + a.gap_bytes + r * 2 * a.stride_bytes;
-            lra_tma_load_1d(dst, src_b, a.core_bytes, fb);
-            lra_tma_load_1d(dst + a.stride_bytes, src_b + a.core_bytes, a.core_bytes, fb);
+            lra_tma_load_1d(sa + slab0 + a.gap_bytes + r * a.stride_bytes, src_b, a.core_bytes, fb);
           }
         }
         if (++slot == (uint32_t)a.nslot) { slot = 0; par ^= 1; }
@@ -123,6 +121,28 @@ __device__ __forceinline__ void lra_region_producer(const lra_region_args& a, co
   }
 }
 
+// The taps of the two pixels this lane owns at one step: {re(e), im(e), re(e + 32), im(e + 32)}.
+struct lra_taps { uint32_t v[4]; };
+
+// Loads of one step (predicated off when the step lies outside the point's chunk range).
+template <int IMM>
+__device__ __forceinline__ void lra_step_load(lra_taps& t, uint32_t addr, uint32_t on) {
+  asm volatile("{\n.reg .pred p;\nsetp.ne.u32 p, %6, 0;\n"
+               "@p ld.shared.v2.b32 {%0, %1}, [%4+%5];\n"
+               "@p ld.shared.v2.b32 {%2, %3}, [%4+%5+256];\n}"
+               : "+r"(t.v[0]), "+r"(t.v[1]), "+r"(t.v[2]), "+r"(t.v[3]) : "r"(addr), "n"(IMM), "r"(on));
+}
+
+// Step mask of a point for consumer warp `warp` of NW: bit s is set iff chunk NW*s + warp lies in the point's chunk
+// range [c_lo, c_hi] (range = c_lo | c_hi << 16, from lra_work.cu).  Warp-uniform.
+template <int NW>
+__device__ __forceinline__ uint32_t lra_step_mask(uint32_t range, int warp) {
+  constexpr int LG = NW == 1 ? 0 : NW == 2 ? 1 : NW == 4 ? 2 : NW == 8 ? 3 : 4;
+  const int c_lo = (int)(range & 0xffffu), c_hi = (int)(range >> 16);
+  const int s_lo = (c_lo - warp + NW - 1) >> LG, s_hi = (c_hi - warp) >> LG;   // s_hi >= s_lo - 1 >= -1
+  return (1u << (s_hi + 1)) - (1u << s_lo);
+}
+
 // Ring set-up shared by the gridder and the degridder: barriers, zeroed slab areas.
 template <int NW>
 __device__ __forceinline__ void lra_region_ring_init(const lra_region_args& a, unsigned char* smem,
@@ -142,17 +162,16 @@ __device__ __forceinline__ void lra_region_ring_init(const lra_region_args& a, u
 
 // Ring geometry of a class for a kernel that keeps `val_bytes` per point in the slot.  Returns false if not even
 // one slot fits (the class then takes the fallback kernels).
-static inline bool lra_region_ring(const lra_geom& q, int val_bytes, lra_region_args* a, int* smem_bytes) {
+static inline bool lra_region_ring(const lra_geom& q, int ngp, bool degrid, int val_bytes, lra_region_args* a, int* smem_bytes) {
   const int slab0 = (LRA_SLOT_VAL + q.per_batch * LRA_RUNMAX * val_bytes + 127) & ~127;
-  const int slot_bytes = (slab0 + 4 * (q.gap + q.per_batch * 2 * q.stride) + 127) & ~127;
-  int nslot = (lra_cta_smem(q.nw, q.ks) - LRA_RING_HDR) / slot_bytes;
+  const int slot_bytes = (slab0 + 8 * (LRA_GAP + q.per_batch * q.stride) + 127) & ~127;
+  int nslot = (lra_cta_smem(q.nw, q.ks, ngp, degrid) - LRA_RING_HDR) / slot_bytes;
   if (nslot < 1) return false;
   if (nslot > 4) nslot = 4;
   a->S = q.S; a->rx = q.rx; a->ry = q.ry; a->ks = q.ks;
-  a->core_bytes = 4 * q.core; a->stride_bytes = 4 * q.stride; a->gap_bytes = 4 * q.gap;
+  a->core_bytes = 8 * q.core; a->stride_bytes = 8 * q.stride; a->gap_bytes = 8 * LRA_GAP;
   a->nslot = nslot; a->slot_bytes = slot_bytes; a->slab0 = slab0;
   a->out_off = LRA_SLOT_VAL + q.per_batch * LRA_RUNMAX * 16;   // degridder: 16 bytes per point come first
   *smem_bytes = LRA_RING_HDR + nslot * slot_bytes;
   return true;
 }
-

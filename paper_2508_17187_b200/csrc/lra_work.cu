@@ -8,10 +8,10 @@
 struct lra_work_args {
   const lra_rec* rec;
   unsigned long long* counters;
-  int shift_x, shift_y, ntx, tile_x, tile_y;
+  int shift_x, shift_y, ntx, tile_x, tile_y, ng;
   uint4* work;
   uint32_t* batch;     // 16 words per batch
-  uint4* pw;           // one 16-byte record per sorted position: {word, k, S, 0}
+  uint4* pw;           // one 16-byte record per sorted position: {word, k, S, c_lo | c_hi << 16}
 };
 
 // exclusive prefix sum over the block (256 threads); returns the block total through `total`
@@ -131,7 +131,7 @@ __global__ void __launch_bounds__(256) lra_work_kernel(const lra_work_args a) {
   for (unsigned j = threadIdx.x; j < n_items_blk; j += 256) {
     const unsigned S = item_sup[j], c = (unsigned)lra_class_of((int)S);
     const unsigned nruns = item_first_run[j + 1] - item_first_run[j];
-    const unsigned per = (unsigned)lra_make_geom((int)S, a.tile_x, a.tile_y).per_batch;
+    const unsigned per = (unsigned)lra_make_geom((int)S, a.tile_x, a.tile_y, a.ng).per_batch;
     const unsigned nb = (nruns + per - 1) / per;
     if (!FILL) {
       atomicAdd(&cls_cnt[0][c], 1u);
@@ -155,7 +155,7 @@ __global__ void __launch_bounds__(256) lra_work_kernel(const lra_work_args a) {
   for (unsigned j = threadIdx.x; j < n_runs_blk; j += 256) {
     const unsigned it = run_item[j], S = item_sup[it], c = (unsigned)lra_class_of((int)S);
     const unsigned first_run = item_first_run[it], nruns = item_first_run[it + 1] - first_run;
-    const unsigned per = (unsigned)lra_make_geom((int)S, a.tile_x, a.tile_y).per_batch;
+    const unsigned per = (unsigned)lra_make_geom((int)S, a.tile_x, a.tile_y, a.ng).per_batch;
     const unsigned q = j - first_run, b = q / per, r = q - b * per;
     uint32_t* rec16 = a.batch + (a.counters[LRA_CNT_BATCH_OFF + c] + item_base[it] + b) * 16ull;
     rec16[4 + r] = a.rec[run_pos[j]].y;
@@ -172,11 +172,13 @@ __global__ void __launch_bounds__(256) lra_work_kernel(const lra_work_args a) {
     const long long i = i0 + e;
     if (i < hi) {
       const unsigned j = my_run[e], it = run_item[j];
-      const lra_geom q = lra_make_geom((int)sp[e], a.tile_x, a.tile_y);
+      const lra_geom q = lra_make_geom((int)sp[e], a.tile_x, a.tile_y, a.ng);
       const unsigned r = (j - item_first_run[it]) % (unsigned)q.per_batch;
       const int ix = rc[e].x & 0xffff, iy = rc[e].x >> 16;
       const int ox = ix - ((ix >> a.shift_x) << a.shift_x), oy = iy - ((iy >> a.shift_y) << a.shift_y);
-      a.pw[i] = make_uint4((unsigned)(4 * (q.gap + (int)r * 2 * q.stride - (oy * q.rx + ox))), rc[e].z, rc[e].w & 0xffu, 0u);
+      const int off = oy * q.rx + ox;
+      a.pw[i] = make_uint4((unsigned)(8 * (LRA_GAP + (int)r * q.stride - off)), rc[e].z, rc[e].w & 0xffu,
+                           (unsigned)(off >> 6) | (unsigned)((off + q.span - 1) >> 6) << 16);
     }
   }
 }
@@ -196,7 +198,7 @@ int lra_build_work(lra_plan* p) {
   const int64_t n = p->npoints;
   if (n == 0) return LRA_OK;
   lra_work_args a;
-  a.rec = p->rec; a.counters = p->counters; a.ntx = p->ntx; a.tile_x = p->tile_x; a.tile_y = p->tile;
+  a.rec = p->rec; a.counters = p->counters; a.ntx = p->ntx; a.tile_x = p->tile_x; a.tile_y = p->tile; a.ng = p->ncorr * p->nterms;
   a.work = nullptr; a.batch = nullptr; a.pw = nullptr;
   a.shift_x = a.shift_y = 0;
   while ((1 << a.shift_x) < p->tile_x) ++a.shift_x;
