@@ -22,8 +22,8 @@ template <int NC>
 __global__ void __launch_bounds__(256)
 lra_degrid_warp_kernel(const lra_rec* __restrict__ rec, const unsigned long long* __restrict__ counters,
                        const float* __restrict__ slabs, const float2* __restrict__ grid, const float* __restrict__ tau,
-                       const float2* vis_in, float2* vis_out, int nchan, int nterms, int nx, int ny, int tile_x, int tile_y,
-                       int ng, int only_fallback) {
+                       const float2* vis_in, float2* vis_out, int nchan, int nterms, int nx, int ny, int tile_x,
+                       lra_fallback_mask fb, int only_fallback) {
   const long long n = (long long)counters[0];
   const size_t plane = (size_t)nx * ny;
   const int lane = threadIdx.x & 31;
@@ -32,7 +32,7 @@ lra_degrid_warp_kernel(const lra_rec* __restrict__ rec, const unsigned long long
   for (long long i = warp0; i < n; i += nwarps) {
     const lra_rec r = rec[i];
     const int ix = r.x & 0xffff, iy = r.x >> 16, S = r.w & 0xff, h = (S - 1) >> 1;
-    if (only_fallback && lra_make_geom(S, tile_x, tile_y, ng).nw != 0) continue;   // the region kernels do those
+    if (only_fallback && !lra_is_fallback(fb, S)) continue;   // the region kernels do those
     const float2* slab = reinterpret_cast<const float2*>(slabs + ((size_t)r.y << 2));
     const unsigned k = r.z;
     const int c = (int)(k % (unsigned)nchan);
@@ -102,8 +102,8 @@ int lra_degrid_impl(lra_plan* p, const float2* grid, const float* tau, const flo
     const int blocks = p->sm_count * 8;
 #define LRA_DG(NC)                                                                                                  \
   lra_degrid_warp_kernel<NC><<<blocks, 256, 0, p->stream>>>(p->rec, p->counters, p->slabs, grid, tau, vis_in, vis_out, \
-                                                            p->nchan, p->nterms, p->nx, p->ny, p->tile_x, p->tile,    \
-                                                            p->ncorr * p->nterms, all_warp ? 0 : 1)
+                                                            p->nchan, p->nterms, p->nx, p->ny, p->tile_x,             \
+                                                            lra_make_fallback_mask(p->tile_x, p->tile, p->ncorr * p->nterms), all_warp ? 0 : 1)
     switch (p->ncorr) {
       case 1: LRA_DG(1); break;
       case 2: LRA_DG(2); break;

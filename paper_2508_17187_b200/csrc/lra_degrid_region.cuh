@@ -19,80 +19,78 @@
 #pragma once
 #include "lra_region.cuh"
 
-// FMAs of one step of one point: the two pixels of this lane on NG grids.  `on` is warp-uniform (a uniform branch).
-template <int NG>
-__device__ __forceinline__ void lra_dstep_fma(lra_u64 (&P1)[NG], lra_u64 (&P2)[NG], const lra_u64 (&G)[2][NG],
-                                              const lra_taps& t, uint32_t on) {
+// One step of the software pipeline: the FMAs of the CURRENT point on the two pixels this lane owns at the step (taps
+// t = {re(e), im(e), re(e + 32), im(e + 32)}), under a uniform branch on `on`, then the loads of the NEXT point's taps
+// for the same step into the same registers.
+template <int NG, int IMM>
+__device__ __forceinline__ void lra_dstep(lra_u64 (&P1)[NG], lra_u64 (&P2)[NG], const lra_u64 (&G)[2][NG], lra_taps& t,
+                                          uint32_t on, uint32_t addr, uint32_t on_next) {
   if constexpr (NG == 1) {
     asm volatile(
-        "{\n.reg .pred p;\n.reg .b64 ar, ai, br, bi;\nsetp.eq.u32 p, %8, 0;\n@p bra.uni SKIP_%=;\n"
-        "mov.b64 ar, {%4, %4};\nmov.b64 ai, {%5, %5};\nmov.b64 br, {%6, %6};\nmov.b64 bi, {%7, %7};\n"
-        "fma.rn.f32x2 %0, ar, %2, %0;\nfma.rn.f32x2 %1, ai, %2, %1;\n"
-        "fma.rn.f32x2 %0, br, %3, %0;\nfma.rn.f32x2 %1, bi, %3, %1;\n"
-        "SKIP_%=:\n}"
-        : "+l"(P1[0]), "+l"(P2[0])
-        : "l"(G[0][0]), "l"(G[1][0]), "r"(t.v[0]), "r"(t.v[1]), "r"(t.v[2]), "r"(t.v[3]), "r"(on));
+        "{\n.reg .pred p, q;\n.reg .b64 ar, ai, br, bi;\nsetp.eq.u32 p, %8, 0;\n@p bra.uni SKIP_%=;\n"
+        "mov.b64 ar, {%2, %2};\nmov.b64 ai, {%3, %3};\nmov.b64 br, {%4, %4};\nmov.b64 bi, {%5, %5};\n"
+        "fma.rn.f32x2 %0, ar, %6, %0;\nfma.rn.f32x2 %1, ai, %6, %1;\n"
+        "fma.rn.f32x2 %0, br, %7, %0;\nfma.rn.f32x2 %1, bi, %7, %1;\n"
+        "SKIP_%=:\nsetp.ne.u32 q, %11, 0;\n"
+        "@q ld.shared.v2.b32 {%2, %3}, [%9+%10];\n@q ld.shared.v2.b32 {%4, %5}, [%9+%10+256];\n}"
+        : "+l"(P1[0]), "+l"(P2[0]), "+r"(t.v[0]), "+r"(t.v[1]), "+r"(t.v[2]), "+r"(t.v[3])
+        : "l"(G[0][0]), "l"(G[1][0]), "r"(on), "r"(addr), "n"(IMM), "r"(on_next));
   }
   if constexpr (NG == 2) {
     asm volatile(
-        "{\n.reg .pred p;\n.reg .b64 ar, ai, br, bi;\nsetp.eq.u32 p, %12, 0;\n@p bra.uni SKIP_%=;\n"
-        "mov.b64 ar, {%8, %8};\nmov.b64 ai, {%9, %9};\nmov.b64 br, {%10, %10};\nmov.b64 bi, {%11, %11};\n"
-        "fma.rn.f32x2 %0, ar, %4, %0;\nfma.rn.f32x2 %2, ai, %4, %2;\n"
-        "fma.rn.f32x2 %1, ar, %5, %1;\nfma.rn.f32x2 %3, ai, %5, %3;\n"
-        "fma.rn.f32x2 %0, br, %6, %0;\nfma.rn.f32x2 %2, bi, %6, %2;\n"
-        "fma.rn.f32x2 %1, br, %7, %1;\nfma.rn.f32x2 %3, bi, %7, %3;\n"
-        "SKIP_%=:\n}"
-        : "+l"(P1[0]), "+l"(P1[1]), "+l"(P2[0]), "+l"(P2[1])
-        : "l"(G[0][0]), "l"(G[0][1]), "l"(G[1][0]), "l"(G[1][1]), "r"(t.v[0]), "r"(t.v[1]), "r"(t.v[2]), "r"(t.v[3]), "r"(on));
+        "{\n.reg .pred p, q;\n.reg .b64 ar, ai, br, bi;\nsetp.eq.u32 p, %12, 0;\n@p bra.uni SKIP_%=;\n"
+        "mov.b64 ar, {%4, %4};\nmov.b64 ai, {%5, %5};\nmov.b64 br, {%6, %6};\nmov.b64 bi, {%7, %7};\n"
+        "fma.rn.f32x2 %0, ar, %8, %0;\nfma.rn.f32x2 %2, ai, %8, %2;\n"
+        "fma.rn.f32x2 %1, ar, %9, %1;\nfma.rn.f32x2 %3, ai, %9, %3;\n"
+        "fma.rn.f32x2 %0, br, %10, %0;\nfma.rn.f32x2 %2, bi, %10, %2;\n"
+        "fma.rn.f32x2 %1, br, %11, %1;\nfma.rn.f32x2 %3, bi, %11, %3;\n"
+        "SKIP_%=:\nsetp.ne.u32 q, %15, 0;\n"
+        "@q ld.shared.v2.b32 {%4, %5}, [%13+%14];\n@q ld.shared.v2.b32 {%6, %7}, [%13+%14+256];\n}"
+        : "+l"(P1[0]), "+l"(P1[1]), "+l"(P2[0]), "+l"(P2[1]), "+r"(t.v[0]), "+r"(t.v[1]), "+r"(t.v[2]), "+r"(t.v[3])
+        : "l"(G[0][0]), "l"(G[0][1]), "l"(G[1][0]), "l"(G[1][1]), "r"(on), "r"(addr), "n"(IMM), "r"(on_next));
   }
   if constexpr (NG == 3) {
     asm volatile(
-        "{\n.reg .pred p;\n.reg .b64 ar, ai, br, bi;\nsetp.eq.u32 p, %16, 0;\n@p bra.uni SKIP_%=;\n"
-        "mov.b64 ar, {%12, %12};\nmov.b64 ai, {%13, %13};\nmov.b64 br, {%14, %14};\nmov.b64 bi, {%15, %15};\n"
-        "fma.rn.f32x2 %0, ar, %6, %0;\nfma.rn.f32x2 %3, ai, %6, %3;\n"
-        "fma.rn.f32x2 %1, ar, %7, %1;\nfma.rn.f32x2 %4, ai, %7, %4;\n"
-        "fma.rn.f32x2 %2, ar, %8, %2;\nfma.rn.f32x2 %5, ai, %8, %5;\n"
-        "fma.rn.f32x2 %0, br, %9, %0;\nfma.rn.f32x2 %3, bi, %9, %3;\n"
-        "fma.rn.f32x2 %1, br, %10, %1;\nfma.rn.f32x2 %4, bi, %10, %4;\n"
-        "fma.rn.f32x2 %2, br, %11, %2;\nfma.rn.f32x2 %5, bi, %11, %5;\n"
-        "SKIP_%=:\n}"
-        : "+l"(P1[0]), "+l"(P1[1]), "+l"(P1[2]), "+l"(P2[0]), "+l"(P2[1]), "+l"(P2[2])
-        : "l"(G[0][0]), "l"(G[0][1]), "l"(G[0][2]), "l"(G[1][0]), "l"(G[1][1]), "l"(G[1][2]), "r"(t.v[0]), "r"(t.v[1]), "r"(t.v[2]), "r"(t.v[3]), "r"(on));
+        "{\n.reg .pred p, q;\n.reg .b64 ar, ai, br, bi;\nsetp.eq.u32 p, %16, 0;\n@p bra.uni SKIP_%=;\n"
+        "mov.b64 ar, {%6, %6};\nmov.b64 ai, {%7, %7};\nmov.b64 br, {%8, %8};\nmov.b64 bi, {%9, %9};\n"
+        "fma.rn.f32x2 %0, ar, %10, %0;\nfma.rn.f32x2 %3, ai, %10, %3;\n"
+        "fma.rn.f32x2 %1, ar, %11, %1;\nfma.rn.f32x2 %4, ai, %11, %4;\n"
+        "fma.rn.f32x2 %2, ar, %12, %2;\nfma.rn.f32x2 %5, ai, %12, %5;\n"
+        "fma.rn.f32x2 %0, br, %13, %0;\nfma.rn.f32x2 %3, bi, %13, %3;\n"
+        "fma.rn.f32x2 %1, br, %14, %1;\nfma.rn.f32x2 %4, bi, %14, %4;\n"
+        "fma.rn.f32x2 %2, br, %15, %2;\nfma.rn.f32x2 %5, bi, %15, %5;\n"
+        "SKIP_%=:\nsetp.ne.u32 q, %19, 0;\n"
+        "@q ld.shared.v2.b32 {%6, %7}, [%17+%18];\n@q ld.shared.v2.b32 {%8, %9}, [%17+%18+256];\n}"
+        : "+l"(P1[0]), "+l"(P1[1]), "+l"(P1[2]), "+l"(P2[0]), "+l"(P2[1]), "+l"(P2[2]), "+r"(t.v[0]), "+r"(t.v[1]), "+r"(t.v[2]), "+r"(t.v[3])
+        : "l"(G[0][0]), "l"(G[0][1]), "l"(G[0][2]), "l"(G[1][0]), "l"(G[1][1]), "l"(G[1][2]), "r"(on), "r"(addr), "n"(IMM), "r"(on_next));
   }
   if constexpr (NG == 4) {
     asm volatile(
-        "{\n.reg .pred p;\n.reg .b64 ar, ai, br, bi;\nsetp.eq.u32 p, %20, 0;\n@p bra.uni SKIP_%=;\n"
-        "mov.b64 ar, {%16, %16};\nmov.b64 ai, {%17, %17};\nmov.b64 br, {%18, %18};\nmov.b64 bi, {%19, %19};\n"
-        "fma.rn.f32x2 %0, ar, %8, %0;\nfma.rn.f32x2 %4, ai, %8, %4;\n"
-        "fma.rn.f32x2 %1, ar, %9, %1;\nfma.rn.f32x2 %5, ai, %9, %5;\n"
-        "fma.rn.f32x2 %2, ar, %10, %2;\nfma.rn.f32x2 %6, ai, %10, %6;\n"
-        "fma.rn.f32x2 %3, ar, %11, %3;\nfma.rn.f32x2 %7, ai, %11, %7;\n"
-        "fma.rn.f32x2 %0, br, %12, %0;\nfma.rn.f32x2 %4, bi, %12, %4;\n"
-        "fma.rn.f32x2 %1, br, %13, %1;\nfma.rn.f32x2 %5, bi, %13, %5;\n"
-        "fma.rn.f32x2 %2, br, %14, %2;\nfma.rn.f32x2 %6, bi, %14, %6;\n"
-        "fma.rn.f32x2 %3, br, %15, %3;\nfma.rn.f32x2 %7, bi, %15, %7;\n"
-        "SKIP_%=:\n}"
-        : "+l"(P1[0]), "+l"(P1[1]), "+l"(P1[2]), "+l"(P1[3]), "+l"(P2[0]), "+l"(P2[1]), "+l"(P2[2]), "+l"(P2[3])
-        : "l"(G[0][0]), "l"(G[0][1]), "l"(G[0][2]), "l"(G[0][3]), "l"(G[1][0]), "l"(G[1][1]), "l"(G[1][2]), "l"(G[1][3]), "r"(t.v[0]), "r"(t.v[1]), "r"(t.v[2]), "r"(t.v[3]), "r"(on));
+        "{\n.reg .pred p, q;\n.reg .b64 ar, ai, br, bi;\nsetp.eq.u32 p, %20, 0;\n@p bra.uni SKIP_%=;\n"
+        "mov.b64 ar, {%8, %8};\nmov.b64 ai, {%9, %9};\nmov.b64 br, {%10, %10};\nmov.b64 bi, {%11, %11};\n"
+        "fma.rn.f32x2 %0, ar, %12, %0;\nfma.rn.f32x2 %4, ai, %12, %4;\n"
+        "fma.rn.f32x2 %1, ar, %13, %1;\nfma.rn.f32x2 %5, ai, %13, %5;\n"
+        "fma.rn.f32x2 %2, ar, %14, %2;\nfma.rn.f32x2 %6, ai, %14, %6;\n"
+        "fma.rn.f32x2 %3, ar, %15, %3;\nfma.rn.f32x2 %7, ai, %15, %7;\n"
+        "fma.rn.f32x2 %0, br, %16, %0;\nfma.rn.f32x2 %4, bi, %16, %4;\n"
+        "fma.rn.f32x2 %1, br, %17, %1;\nfma.rn.f32x2 %5, bi, %17, %5;\n"
+        "fma.rn.f32x2 %2, br, %18, %2;\nfma.rn.f32x2 %6, bi, %18, %6;\n"
+        "fma.rn.f32x2 %3, br, %19, %3;\nfma.rn.f32x2 %7, bi, %19, %7;\n"
+        "SKIP_%=:\nsetp.ne.u32 q, %23, 0;\n"
+        "@q ld.shared.v2.b32 {%8, %9}, [%21+%22];\n@q ld.shared.v2.b32 {%10, %11}, [%21+%22+256];\n}"
+        : "+l"(P1[0]), "+l"(P1[1]), "+l"(P1[2]), "+l"(P1[3]), "+l"(P2[0]), "+l"(P2[1]), "+l"(P2[2]), "+l"(P2[3]), "+r"(t.v[0]), "+r"(t.v[1]), "+r"(t.v[2]), "+r"(t.v[3])
+        : "l"(G[0][0]), "l"(G[0][1]), "l"(G[0][2]), "l"(G[0][3]), "l"(G[1][0]), "l"(G[1][1]), "l"(G[1][2]), "l"(G[1][3]), "r"(on), "r"(addr), "n"(IMM), "r"(on_next));
   }
 }
 
-template <int NW, int NG, int KS, int B, int E>
-struct lra_dsteps {
-  static __device__ __forceinline__ void load(lra_taps (&T)[KS], uint32_t addr, uint32_t mask) {
-    if constexpr (B < E) {
-      lra_step_load<B * 512 * NW>(T[B], addr, mask & (1u << B));
-      lra_dsteps<NW, NG, KS, B + 1, E>::load(T, addr, mask);
-    }
+template <int NW, int NG, int KS, int B>
+__device__ __forceinline__ void lra_drun_steps(lra_u64 (&P1)[NG], lra_u64 (&P2)[NG], const lra_u64 (&G)[KS][2][NG],
+                                               lra_taps (&T)[KS], uint32_t mask, uint32_t addr_next, uint32_t mask_next) {
+  if constexpr (B < KS) {
+    lra_dstep<NG, B * 512 * NW>(P1, P2, G[B], T[B], mask & (1u << B), addr_next, mask_next & (1u << B));
+    lra_drun_steps<NW, NG, KS, B + 1>(P1, P2, G, T, mask, addr_next, mask_next);
   }
-  static __device__ __forceinline__ void fma(lra_u64 (&P1)[NG], lra_u64 (&P2)[NG], const lra_u64 (&G)[KS][2][NG],
-                                             const lra_taps (&T)[KS], uint32_t mask) {
-    if constexpr (B < E) {
-      lra_dstep_fma<NG>(P1, P2, G[B], T[B], mask & (1u << B));
-      lra_dsteps<NW, NG, KS, B + 1, E>::fma(P1, P2, G, T, mask);
-    }
-  }
-};
+}
 
 template <int NW, int KS, int NG>
 __global__ void __launch_bounds__((NW + 1) * 32) __maxnreg__(LRA_MAXNREG(NW, KS, NG, true)) lra_degrid_region_kernel(const lra_region_args a) {
@@ -107,7 +105,6 @@ __global__ void __launch_bounds__((NW + 1) * 32) __maxnreg__(LRA_MAXNREG(NW, KS,
     return;
   }
   // -------------------------------------------------------------------- consumer warps
-  constexpr int KA = (KS + 1) / 2;
   constexpr int V = NG == 1 ? 8 : NG == 2 ? 16 : 32;   // values of four points (2 * NG each), padded to a power of two
   lra_u64 G[KS][2][NG];   // the region of the model grid: (re, im) of the lane's two pixels at every step
   lra_taps T[KS];
@@ -149,8 +146,8 @@ __global__ void __launch_bounds__((NW + 1) * 32) __maxnreg__(LRA_MAXNREG(NW, KS,
     float* out = reinterpret_cast<float*>(sp + a.out_off);
     // software pipeline over the points of the batch (as in the gridder), four points per reduction
     uint4 pc = *reinterpret_cast<const uint4*>(rec);
-    uint32_t cur_addr = lane_base + pc.x, cur_mask = count ? lra_step_mask<NW>(pc.w, warp) : 0u;
-    lra_dsteps<NW, NG, KS, 0, KA>::load(T, cur_addr, cur_mask);
+    uint32_t mask = count ? lra_step_mask<NW>(pc.w, warp) : 0u;
+    lra_load_steps<NW, KS, 0>(T, lane_base + pc.x, mask);
     for (unsigned q0 = 0; q0 < count; q0 += 4) {
       float v[V];
 #pragma unroll
@@ -158,15 +155,12 @@ __global__ void __launch_bounds__((NW + 1) * 32) __maxnreg__(LRA_MAXNREG(NW, KS,
 #pragma unroll
       for (int u = 0; u < 4; ++u) {
         rec += 16;
-        const uint4 pn = *reinterpret_cast<const uint4*>(rec);
-        const uint32_t nxt_addr = lane_base + pn.x, nxt_mask = q0 + u + 1 < count ? lra_step_mask<NW>(pn.w, warp) : 0u;
+        pc = *reinterpret_cast<const uint4*>(rec);
+        const uint32_t addr_next = lane_base + pc.x, mask_next = q0 + u + 1 < count ? lra_step_mask<NW>(pc.w, warp) : 0u;
         lra_u64 P1[NG], P2[NG];
 #pragma unroll
         for (int g = 0; g < NG; ++g) P1[g] = P2[g] = 0ull;
-        lra_dsteps<NW, NG, KS, KA, KS>::load(T, cur_addr, cur_mask);
-        lra_dsteps<NW, NG, KS, 0, KA>::fma(P1, P2, G, T, cur_mask);
-        lra_dsteps<NW, NG, KS, 0, KA>::load(T, nxt_addr, nxt_mask);
-        lra_dsteps<NW, NG, KS, KA, KS>::fma(P1, P2, G, T, cur_mask);
+        lra_drun_steps<NW, NG, KS, 0>(P1, P2, G, T, mask, addr_next, mask_next);
 #pragma unroll
         for (int g = 0; g < NG; ++g) {   // conj(c) * G = (cre*Gre + cim*Gim) + i (cre*Gim - cim*Gre)
           float p1r, p1i, p2r, p2i;
@@ -175,7 +169,7 @@ __global__ void __launch_bounds__((NW + 1) * 32) __maxnreg__(LRA_MAXNREG(NW, KS,
           v[(u * NG + g) * 2 + 0] = p1r + p2i;
           v[(u * NG + g) * 2 + 1] = p1i - p2r;
         }
-        cur_addr = nxt_addr; cur_mask = nxt_mask;
+        mask = mask_next;
       }
       // transposing butterfly: afterwards lane l holds the warp total of value l % V
 #pragma unroll
@@ -192,8 +186,7 @@ __global__ void __launch_bounds__((NW + 1) * 32) __maxnreg__(LRA_MAXNREG(NW, KS,
       const unsigned left = count - q0;
       if (lane < 8 * NG && (unsigned)(lane / (2 * NG)) < left) atomicAdd(out + q0 * (2 * NG) + lane, v[0]);
     }
-    __syncwarp();
-    if (lane == 0) lra_mbar_arrive(empty0 + 8 * slot);
+    lra_mbar_arrive(empty0 + 8 * slot);   // every lane, after its own reads of the slot: no divergent branch in the loop
     if (h.y & LRA_BATCH_LAST) fresh = true;
     if (h.y & LRA_BATCH_END) break;
     if (++slot == (uint32_t)a.nslot) { slot = 0; par ^= 1; }

@@ -62,13 +62,13 @@ __global__ void __launch_bounds__(256)
 lra_grid_atomic_kernel(const lra_rec* __restrict__ rec, const unsigned long long* __restrict__ counters,
                        const float* __restrict__ slabs, const float2* __restrict__ vis, const float* __restrict__ wt,
                        const float* __restrict__ tau, int nchan, int ncorr, int nterms, int nx, int ny,
-                       int tile_x, int tile_y, int ng, int only_fallback, float2* __restrict__ grid) {
+                       int tile_x, lra_fallback_mask fb, int only_fallback, float2* __restrict__ grid) {
   const long long n = (long long)counters[0];
   const size_t plane = (size_t)nx * ny;
   for (long long i = blockIdx.x; i < n; i += gridDim.x) {
     const lra_rec r = rec[i];
     const int ix = r.x & 0xffff, iy = r.x >> 16, S = r.w & 0xff, h = (S - 1) >> 1;
-    if (only_fallback && lra_make_geom(S, tile_x, tile_y, ng).nw != 0) continue;   // the region kernels do those
+    if (only_fallback && !lra_is_fallback(fb, S)) continue;   // the region kernels do those
     const float2* slab = reinterpret_cast<const float2*>(slabs + ((size_t)r.y << 2));
     const uint32_t k = r.z;
     const int c = (int)(k % (uint32_t)nchan);
@@ -120,7 +120,7 @@ int lra_grid_impl(lra_plan* p, const float2* vis, const float* wt, const float* 
   if (all_atomic || fallback) {  // regions that fit no group of the region kernel (or the "before" variant)
     lra_grid_atomic_kernel<<<p->sm_count * 16, 256, 0, p->stream>>>(p->rec, p->counters, p->slabs, vis, wt, tau,
                                                                      p->nchan, p->ncorr, p->nterms, p->nx, p->ny,
-                                                                     p->tile_x, p->tile, p->ncorr * p->nterms, all_atomic ? 0 : 1, grid);
+                                                                     p->tile_x, lra_make_fallback_mask(p->tile_x, p->tile, p->ncorr * p->nterms), all_atomic ? 0 : 1, grid);
     LRA_LAUNCH_CHECK(p);
     if (all_atomic) return LRA_OK;
   }

@@ -19,14 +19,16 @@
 //   * A point's taps lie in the pixel range [off, off + L): a warp runs only its steps inside that range.  The step
 //     mask of a point is warp-uniform and lives in uniform registers, so a skipped step costs one uniform branch and
 //     two predicated-off loads, no FMA-pipe time: the rows of the region above and below the footprint are free.
+//     (Measured alternative, rejected: one indirect jump per point to straight-line code of its step range; fewer
+//     instructions, but the jump's latency made it 10 % slower.)
 //   * The tap update of one pixel on one grid is two FFMA2 (fma.rn.f32x2) with the tap as the scalar operand:
 //       acc(re, im) += cre * (vx, vy);   acc(re, im) += cim * (-vy, vx)
 //     (ptxas folds the duplicated tap into the FFMA2's scalar-broadcast operand form), so two 8-byte loads feed
 //     4 * NG FFMA2: the FP32 pipe and the shared-memory port saturate together at NG = 2 and the pipe alone binds at
 //     NG = 4.
-//   * The loads of a point are issued half a point ahead of the FMAs that use them (two halves of the step range, taps
-//     of one half in flight while the other half multiplies), by hand: the branches around the steps keep the
-//     compiler from doing it.
+//   * The loads are software-pipelined by hand (the branches around the steps keep the compiler from doing it): a
+//     step multiplies the taps of point q and then reloads the same registers with the taps of point q + 1, so a
+//     tap is in flight for a whole point.
 //   * lra_prepare_kernel first gathers vis / weight in SORTED order and writes, per point, the NG operand pairs
 //     (vx, vy, -vy, vx) = wt*tau*V and the point's slab offset and chunk range as one contiguous record.
 //   * The producer warp walks the batch stream of lra_work.cu and issues, per batch (= up to 12 slab runs of an
@@ -37,103 +39,79 @@
 #pragma once
 #include "lra_region.cuh"
 
-// FMAs of one step: the two pixels of this lane on NG grids, acc[pixel][grid] = (re, im).  `on` is warp-uniform: a
-// real (uniform) branch over the block.
-template <int NG>
-__device__ __forceinline__ void lra_step_fma(lra_u64 (&acc)[2][NG], const lra_u64 (&V)[NG], const lra_u64 (&W)[NG],
-                                             const lra_taps& t, uint32_t on) {
+// One step of the software pipeline: the FMAs of the CURRENT point on the two pixels this lane owns at the step
+// (acc[pixel][grid] = (re, im), taps t = {re(e), im(e), re(e + 32), im(e + 32)}), under a uniform branch on `on`, then
+// the loads of the NEXT point's taps for the same step into the same registers (predicated on `on_next`): the taps
+// of a step are in flight for one whole point.
+template <int NG, int IMM>
+__device__ __forceinline__ void lra_step(lra_u64 (&acc)[2][NG], const lra_u64 (&V)[NG], const lra_u64 (&W)[NG], lra_taps& t,
+                                         uint32_t on, uint32_t addr, uint32_t on_next) {
   if constexpr (NG == 1) {
     asm volatile(
-        "{\n.reg .pred p;\n.reg .b64 ar, ai, br, bi;\nsetp.eq.u32 p, %8, 0;\n@p bra.uni SKIP_%=;\n"
-        "mov.b64 ar, {%4, %4};\nmov.b64 ai, {%5, %5};\nmov.b64 br, {%6, %6};\nmov.b64 bi, {%7, %7};\n"
-        "fma.rn.f32x2 %0, ar, %2, %0;\nfma.rn.f32x2 %1, br, %2, %1;\n"
-        "fma.rn.f32x2 %0, ai, %3, %0;\nfma.rn.f32x2 %1, bi, %3, %1;\n"
-        "SKIP_%=:\n}"
-        : "+l"(acc[0][0]), "+l"(acc[1][0])
-        : "l"(V[0]), "l"(W[0]), "r"(t.v[0]), "r"(t.v[1]), "r"(t.v[2]), "r"(t.v[3]), "r"(on));
+        "{\n.reg .pred p, q;\n.reg .b64 ar, ai, br, bi;\nsetp.eq.u32 p, %8, 0;\n@p bra.uni SKIP_%=;\n"
+        "mov.b64 ar, {%2, %2};\nmov.b64 ai, {%3, %3};\nmov.b64 br, {%4, %4};\nmov.b64 bi, {%5, %5};\n"
+        "fma.rn.f32x2 %0, ar, %6, %0;\nfma.rn.f32x2 %1, br, %6, %1;\n"
+        "fma.rn.f32x2 %0, ai, %7, %0;\nfma.rn.f32x2 %1, bi, %7, %1;\n"
+        "SKIP_%=:\nsetp.ne.u32 q, %11, 0;\n"
+        "@q ld.shared.v2.b32 {%2, %3}, [%9+%10];\n@q ld.shared.v2.b32 {%4, %5}, [%9+%10+256];\n}"
+        : "+l"(acc[0][0]), "+l"(acc[1][0]), "+r"(t.v[0]), "+r"(t.v[1]), "+r"(t.v[2]), "+r"(t.v[3])
+        : "l"(V[0]), "l"(W[0]), "r"(on), "r"(addr), "n"(IMM), "r"(on_next));
   }
   if constexpr (NG == 2) {
     asm volatile(
-        "{\n.reg .pred p;\n.reg .b64 ar, ai, br, bi;\nsetp.eq.u32 p, %12, 0;\n@p bra.uni SKIP_%=;\n"
-        "mov.b64 ar, {%8, %8};\nmov.b64 ai, {%9, %9};\nmov.b64 br, {%10, %10};\nmov.b64 bi, {%11, %11};\n"
-        "fma.rn.f32x2 %0, ar, %4, %0;\nfma.rn.f32x2 %1, ar, %6, %1;\n"
-        "fma.rn.f32x2 %2, br, %4, %2;\nfma.rn.f32x2 %3, br, %6, %3;\n"
-        "fma.rn.f32x2 %0, ai, %5, %0;\nfma.rn.f32x2 %1, ai, %7, %1;\n"
-        "fma.rn.f32x2 %2, bi, %5, %2;\nfma.rn.f32x2 %3, bi, %7, %3;\n"
-        "SKIP_%=:\n}"
-        : "+l"(acc[0][0]), "+l"(acc[0][1]), "+l"(acc[1][0]), "+l"(acc[1][1])
-        : "l"(V[0]), "l"(W[0]), "l"(V[1]), "l"(W[1]), "r"(t.v[0]), "r"(t.v[1]), "r"(t.v[2]), "r"(t.v[3]), "r"(on));
+        "{\n.reg .pred p, q;\n.reg .b64 ar, ai, br, bi;\nsetp.eq.u32 p, %12, 0;\n@p bra.uni SKIP_%=;\n"
+        "mov.b64 ar, {%4, %4};\nmov.b64 ai, {%5, %5};\nmov.b64 br, {%6, %6};\nmov.b64 bi, {%7, %7};\n"
+        "fma.rn.f32x2 %0, ar, %8, %0;\nfma.rn.f32x2 %1, ar, %10, %1;\n"
+        "fma.rn.f32x2 %2, br, %8, %2;\nfma.rn.f32x2 %3, br, %10, %3;\n"
+        "fma.rn.f32x2 %0, ai, %9, %0;\nfma.rn.f32x2 %1, ai, %11, %1;\n"
+        "fma.rn.f32x2 %2, bi, %9, %2;\nfma.rn.f32x2 %3, bi, %11, %3;\n"
+        "SKIP_%=:\nsetp.ne.u32 q, %15, 0;\n"
+        "@q ld.shared.v2.b32 {%4, %5}, [%13+%14];\n@q ld.shared.v2.b32 {%6, %7}, [%13+%14+256];\n}"
+        : "+l"(acc[0][0]), "+l"(acc[0][1]), "+l"(acc[1][0]), "+l"(acc[1][1]), "+r"(t.v[0]), "+r"(t.v[1]), "+r"(t.v[2]), "+r"(t.v[3])
+        : "l"(V[0]), "l"(W[0]), "l"(V[1]), "l"(W[1]), "r"(on), "r"(addr), "n"(IMM), "r"(on_next));
   }
   if constexpr (NG == 3) {
     asm volatile(
-        "{\n.reg .pred p;\n.reg .b64 ar, ai, br, bi;\nsetp.eq.u32 p, %16, 0;\n@p bra.uni SKIP_%=;\n"
-        "mov.b64 ar, {%12, %12};\nmov.b64 ai, {%13, %13};\nmov.b64 br, {%14, %14};\nmov.b64 bi, {%15, %15};\n"
-        "fma.rn.f32x2 %0, ar, %6, %0;\nfma.rn.f32x2 %1, ar, %8, %1;\n"
-        "fma.rn.f32x2 %2, ar, %10, %2;\nfma.rn.f32x2 %3, br, %6, %3;\n"
-        "fma.rn.f32x2 %4, br, %8, %4;\nfma.rn.f32x2 %5, br, %10, %5;\n"
-        "fma.rn.f32x2 %0, ai, %7, %0;\nfma.rn.f32x2 %1, ai, %9, %1;\n"
-        "fma.rn.f32x2 %2, ai, %11, %2;\nfma.rn.f32x2 %3, bi, %7, %3;\n"
-        "fma.rn.f32x2 %4, bi, %9, %4;\nfma.rn.f32x2 %5, bi, %11, %5;\n"
-        "SKIP_%=:\n}"
-        : "+l"(acc[0][0]), "+l"(acc[0][1]), "+l"(acc[0][2]), "+l"(acc[1][0]), "+l"(acc[1][1]), "+l"(acc[1][2])
-        : "l"(V[0]), "l"(W[0]), "l"(V[1]), "l"(W[1]), "l"(V[2]), "l"(W[2]), "r"(t.v[0]), "r"(t.v[1]), "r"(t.v[2]), "r"(t.v[3]), "r"(on));
+        "{\n.reg .pred p, q;\n.reg .b64 ar, ai, br, bi;\nsetp.eq.u32 p, %16, 0;\n@p bra.uni SKIP_%=;\n"
+        "mov.b64 ar, {%6, %6};\nmov.b64 ai, {%7, %7};\nmov.b64 br, {%8, %8};\nmov.b64 bi, {%9, %9};\n"
+        "fma.rn.f32x2 %0, ar, %10, %0;\nfma.rn.f32x2 %1, ar, %12, %1;\n"
+        "fma.rn.f32x2 %2, ar, %14, %2;\nfma.rn.f32x2 %3, br, %10, %3;\n"
+        "fma.rn.f32x2 %4, br, %12, %4;\nfma.rn.f32x2 %5, br, %14, %5;\n"
+        "fma.rn.f32x2 %0, ai, %11, %0;\nfma.rn.f32x2 %1, ai, %13, %1;\n"
+        "fma.rn.f32x2 %2, ai, %15, %2;\nfma.rn.f32x2 %3, bi, %11, %3;\n"
+        "fma.rn.f32x2 %4, bi, %13, %4;\nfma.rn.f32x2 %5, bi, %15, %5;\n"
+        "SKIP_%=:\nsetp.ne.u32 q, %19, 0;\n"
+        "@q ld.shared.v2.b32 {%6, %7}, [%17+%18];\n@q ld.shared.v2.b32 {%8, %9}, [%17+%18+256];\n}"
+        : "+l"(acc[0][0]), "+l"(acc[0][1]), "+l"(acc[0][2]), "+l"(acc[1][0]), "+l"(acc[1][1]), "+l"(acc[1][2]), "+r"(t.v[0]), "+r"(t.v[1]), "+r"(t.v[2]), "+r"(t.v[3])
+        : "l"(V[0]), "l"(W[0]), "l"(V[1]), "l"(W[1]), "l"(V[2]), "l"(W[2]), "r"(on), "r"(addr), "n"(IMM), "r"(on_next));
   }
   if constexpr (NG == 4) {
     asm volatile(
-        "{\n.reg .pred p;\n.reg .b64 ar, ai, br, bi;\nsetp.eq.u32 p, %20, 0;\n@p bra.uni SKIP_%=;\n"
-        "mov.b64 ar, {%16, %16};\nmov.b64 ai, {%17, %17};\nmov.b64 br, {%18, %18};\nmov.b64 bi, {%19, %19};\n"
-        "fma.rn.f32x2 %0, ar, %8, %0;\nfma.rn.f32x2 %1, ar, %10, %1;\n"
-        "fma.rn.f32x2 %2, ar, %12, %2;\nfma.rn.f32x2 %3, ar, %14, %3;\n"
-        "fma.rn.f32x2 %4, br, %8, %4;\nfma.rn.f32x2 %5, br, %10, %5;\n"
-        "fma.rn.f32x2 %6, br, %12, %6;\nfma.rn.f32x2 %7, br, %14, %7;\n"
-        "fma.rn.f32x2 %0, ai, %9, %0;\nfma.rn.f32x2 %1, ai, %11, %1;\n"
-        "fma.rn.f32x2 %2, ai, %13, %2;\nfma.rn.f32x2 %3, ai, %15, %3;\n"
-        "fma.rn.f32x2 %4, bi, %9, %4;\nfma.rn.f32x2 %5, bi, %11, %5;\n"
-        "fma.rn.f32x2 %6, bi, %13, %6;\nfma.rn.f32x2 %7, bi, %15, %7;\n"
-        "SKIP_%=:\n}"
-        : "+l"(acc[0][0]), "+l"(acc[0][1]), "+l"(acc[0][2]), "+l"(acc[0][3]), "+l"(acc[1][0]), "+l"(acc[1][1]), "+l"(acc[1][2]), "+l"(acc[1][3])
-        : "l"(V[0]), "l"(W[0]), "l"(V[1]), "l"(W[1]), "l"(V[2]), "l"(W[2]), "l"(V[3]), "l"(W[3]), "r"(t.v[0]), "r"(t.v[1]), "r"(t.v[2]), "r"(t.v[3]), "r"(on));
+        "{\n.reg .pred p, q;\n.reg .b64 ar, ai, br, bi;\nsetp.eq.u32 p, %20, 0;\n@p bra.uni SKIP_%=;\n"
+        "mov.b64 ar, {%8, %8};\nmov.b64 ai, {%9, %9};\nmov.b64 br, {%10, %10};\nmov.b64 bi, {%11, %11};\n"
+        "fma.rn.f32x2 %0, ar, %12, %0;\nfma.rn.f32x2 %1, ar, %14, %1;\n"
+        "fma.rn.f32x2 %2, ar, %16, %2;\nfma.rn.f32x2 %3, ar, %18, %3;\n"
+        "fma.rn.f32x2 %4, br, %12, %4;\nfma.rn.f32x2 %5, br, %14, %5;\n"
+        "fma.rn.f32x2 %6, br, %16, %6;\nfma.rn.f32x2 %7, br, %18, %7;\n"
+        "fma.rn.f32x2 %0, ai, %13, %0;\nfma.rn.f32x2 %1, ai, %15, %1;\n"
+        "fma.rn.f32x2 %2, ai, %17, %2;\nfma.rn.f32x2 %3, ai, %19, %3;\n"
+        "fma.rn.f32x2 %4, bi, %13, %4;\nfma.rn.f32x2 %5, bi, %15, %5;\n"
+        "fma.rn.f32x2 %6, bi, %17, %6;\nfma.rn.f32x2 %7, bi, %19, %7;\n"
+        "SKIP_%=:\nsetp.ne.u32 q, %23, 0;\n"
+        "@q ld.shared.v2.b32 {%8, %9}, [%21+%22];\n@q ld.shared.v2.b32 {%10, %11}, [%21+%22+256];\n}"
+        : "+l"(acc[0][0]), "+l"(acc[0][1]), "+l"(acc[0][2]), "+l"(acc[0][3]), "+l"(acc[1][0]), "+l"(acc[1][1]), "+l"(acc[1][2]), "+l"(acc[1][3]), "+r"(t.v[0]), "+r"(t.v[1]), "+r"(t.v[2]), "+r"(t.v[3])
+        : "l"(V[0]), "l"(W[0]), "l"(V[1]), "l"(W[1]), "l"(V[2]), "l"(W[2]), "l"(V[3]), "l"(W[3]), "r"(on), "r"(addr), "n"(IMM), "r"(on_next));
   }
 }
 
-// Steps [B, E) of a point, unrolled: loads and FMAs.
-template <int NW, int NG, int KS, int B, int E>
-struct lra_steps {
-  static __device__ __forceinline__ void load(lra_taps (&T)[KS], uint32_t addr, uint32_t mask) {
-    if constexpr (B < E) {
-      lra_step_load<B * 512 * NW>(T[B], addr, mask & (1u << B));
-      lra_steps<NW, NG, KS, B + 1, E>::load(T, addr, mask);
-    }
+// Steps [B, KS) of a point, unrolled.
+template <int NW, int NG, int KS, int B>
+__device__ __forceinline__ void lra_run_steps(lra_u64 (&acc)[KS][2][NG], const lra_u64 (&V)[NG], const lra_u64 (&W)[NG],
+                                              lra_taps (&T)[KS], uint32_t mask, uint32_t addr_next, uint32_t mask_next) {
+  if constexpr (B < KS) {
+    lra_step<NG, B * 512 * NW>(acc[B], V, W, T[B], mask & (1u << B), addr_next, mask_next & (1u << B));
+    lra_run_steps<NW, NG, KS, B + 1>(acc, V, W, T, mask, addr_next, mask_next);
   }
-  static __device__ __forceinline__ void fma(lra_u64 (&acc)[KS][2][NG], const lra_u64 (&V)[NG], const lra_u64 (&W)[NG],
-                                             const lra_taps (&T)[KS], uint32_t mask) {
-    if constexpr (B < E) {
-      lra_step_fma<NG>(acc[B], V, W, T[B], mask & (1u << B));
-      lra_steps<NW, NG, KS, B + 1, E>::fma(acc, V, W, T, mask);
-    }
-  }
-};
-
-// One point as a consumer warp sees it: operand pairs per grid, address of the lane's first tap, step mask.
-template <int NG>
-struct lra_point {
-  lra_u64 V[NG], W[NG];   // (vx, vy), (-vy, vx)
-  uint32_t addr, mask;
-};
-// rec: the point's record in the slot (lra_point_bytes); lane_base: shared-memory address of the slot's slab area
-// + 8 * (64 * warp + lane).  mask bit s is set iff chunk NW*s + warp lies in the point's chunk range [c_lo, c_hi].
-template <int NW, int NG>
-__device__ __forceinline__ lra_point<NG> lra_get_point(const unsigned char* rec, uint32_t lane_base, int warp, bool valid) {
-  lra_point<NG> p;
-#pragma unroll
-  for (int g = 0; g < NG; ++g) {
-    const ulonglong2 v = *reinterpret_cast<const ulonglong2*>(rec + 16 * g);
-    p.V[g] = v.x; p.W[g] = v.y;
-  }
-  const uint2 wc = *reinterpret_cast<const uint2*>(rec + 16 * NG);
-  p.mask = valid ? lra_step_mask<NW>(wc.y, warp) : 0u;
-  p.addr = lane_base + wc.x;
-  return p;
 }
 
 template <int NW, int KS, int NG>
@@ -150,7 +128,6 @@ __global__ void __launch_bounds__((NW + 1) * 32) __maxnreg__(LRA_MAXNREG(NW, KS,
     return;
   }
   // -------------------------------------------------------------------- consumer warps
-  constexpr int KA = (KS + 1) / 2;   // steps [0, KA): first half, [KA, KS): second half
   lra_u64 acc[KS][2][NG];
 #pragma unroll
   for (int s = 0; s < KS; ++s)
@@ -168,20 +145,25 @@ __global__ void __launch_bounds__((NW + 1) * 32) __maxnreg__(LRA_MAXNREG(NW, KS,
     const unsigned count = h.y & 0xff;
     const uint32_t lane_base = slots0 + slot * a.slot_bytes + lane_off;
     const unsigned char* rec = sp + LRA_SLOT_VAL;
-    // software pipeline over the points of the batch: the loads of a half are in flight while the other half multiplies
-    lra_point<NG> cur = lra_get_point<NW, NG>(rec, lane_base, warp, count > 0);
-    lra_steps<NW, NG, KS, 0, KA>::load(T, cur.addr, cur.mask);
+    // software pipeline over the points of the batch: while a step multiplies the taps of point q it reloads its tap
+    // registers for point q + 1; the record of point q + 1 is read while point q runs
+    uint2 wc = *reinterpret_cast<const uint2*>(rec + 16 * NG);
+    uint32_t mask = count ? lra_step_mask<NW>(wc.y, warp) : 0u;
+    lra_load_steps<NW, KS, 0>(T, lane_base + wc.x, mask);
     for (unsigned q = 0; q < count; ++q) {
+      lra_u64 V[NG], W[NG];
+#pragma unroll
+      for (int g = 0; g < NG; ++g) {
+        const ulonglong2 v = *reinterpret_cast<const ulonglong2*>(rec + 16 * g);
+        V[g] = v.x; W[g] = v.y;
+      }
       rec += PB;
-      const lra_point<NG> nxt = lra_get_point<NW, NG>(rec, lane_base, warp, q + 1 < count);
-      lra_steps<NW, NG, KS, KA, KS>::load(T, cur.addr, cur.mask);
-      lra_steps<NW, NG, KS, 0, KA>::fma(acc, cur.V, cur.W, T, cur.mask);
-      lra_steps<NW, NG, KS, 0, KA>::load(T, nxt.addr, nxt.mask);
-      lra_steps<NW, NG, KS, KA, KS>::fma(acc, cur.V, cur.W, T, cur.mask);
-      cur = nxt;
+      wc = *reinterpret_cast<const uint2*>(rec + 16 * NG);
+      const uint32_t addr_next = lane_base + wc.x, mask_next = q + 1 < count ? lra_step_mask<NW>(wc.y, warp) : 0u;
+      lra_run_steps<NW, NG, KS, 0>(acc, V, W, T, mask, addr_next, mask_next);
+      mask = mask_next;
     }
-    __syncwarp();
-    if (lane == 0) lra_mbar_arrive(empty0 + 8 * slot);
+    lra_mbar_arrive(empty0 + 8 * slot);   // every lane, after its own reads of the slot: no divergent branch in the loop
     if (h.y & LRA_BATCH_LAST) {
       // ---- row a4: add the item's region to the grid, once ----
       const int hh = (a.S - 1) >> 1;

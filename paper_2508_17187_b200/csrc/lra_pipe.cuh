@@ -52,8 +52,8 @@ __host__ __device__ constexpr int lra_grids_per_pass(int ng) { return ng < LRA_N
 // all the registers that this number of CTAs leaves (lra_regs).
 __host__ __device__ constexpr int lra_regs_need(int ks, int ngp, bool degrid) {
   // rows: grids per pass 1..4; columns: KS 1..8
-  constexpr int G[4][8] = {{48, 48, 56, 64, 80, 80, 104, 104}, {48, 56, 64, 80, 120, 120, 120, 120}, {64, 72, 88, 112, 112, 112, 112, 112}, {80, 96, 120, 136, 136, 136, 136, 136}};
-  constexpr int D[4][8] = {{48, 56, 56, 64, 80, 80, 96, 96}, {56, 64, 64, 80, 112, 112, 112, 112}, {64, 80, 96, 112, 112, 112, 112, 112}, {72, 104, 120, 136, 136, 136, 136, 136}};
+  constexpr int G[4][8] = {{48, 48, 56, 64, 80, 80, 104, 104}, {48, 56, 64, 80, 96, 96, 96, 96}, {64, 72, 88, 112, 112, 112, 112, 112}, {80, 96, 120, 136, 136, 136, 136, 136}};
+  constexpr int D[4][8] = {{48, 56, 56, 64, 80, 80, 96, 96}, {56, 64, 64, 80, 96, 96, 96, 96}, {64, 80, 96, 112, 112, 112, 112, 112}, {72, 104, 120, 136, 136, 136, 136, 136}};
   return degrid ? D[ngp - 1][ks - 1] : G[ngp - 1][ks - 1];
 }
 // The register file is 16384 registers per SM sub-partition and the warps of the resident CTAs are dealt round to the
@@ -104,6 +104,19 @@ __host__ __device__ inline lra_geom lra_make_geom(int S, int tile_x, int tile_y,
   return q;
 }
 __host__ __device__ inline int lra_class_of(int S) { return (S - 1) >> 1; }
+// Which support classes take the fallback kernels (bit c of lo for c < 64, bit c - 64 of hi): computed once on the
+// host, so that per-point kernels need not evaluate the geometry.
+struct lra_fallback_mask { unsigned long long lo; unsigned hi; };
+inline lra_fallback_mask lra_make_fallback_mask(int tile_x, int tile_y, int ng) {
+  lra_fallback_mask m = {0ull, 0u};
+  for (int c = 0; c < LRA_NCLASS; ++c)
+    if (lra_make_geom(2 * c + 1, tile_x, tile_y, ng).nw == 0) { if (c < 64) m.lo |= 1ull << c; else m.hi |= 1u << (c - 64); }
+  return m;
+}
+__device__ __forceinline__ bool lra_is_fallback(const lra_fallback_mask& m, int S) {
+  const int c = lra_class_of(S);
+  return c < 64 ? (m.lo >> c) & 1ull : (m.hi >> (c - 64)) & 1u;
+}
 
 // ---------------------------------------------------------------------------------------------------
 // Batch stream (built once per lra_bin by lra_work.cu; geometry only, reused by every lra_grid / lra_degrid).

@@ -142,13 +142,21 @@ __device__ __forceinline__ uint32_t lra_step_mask(uint32_t range, int warp) {
   const int s_lo = (c_lo - warp + NW - 1) >> LG, s_hi = (c_hi - warp) >> LG;   // s_hi >= s_lo - 1 >= -1
   return (1u << (s_hi + 1)) - (1u << s_lo);
 }
+// The tap loads of a point, steps [B, KS): predicated on the bits of `mask`.
+template <int NW, int KS, int B>
+__device__ __forceinline__ void lra_load_steps(lra_taps (&T)[KS], uint32_t addr, uint32_t mask) {
+  if constexpr (B < KS) {
+    lra_step_load<B * 512 * NW>(T[B], addr, mask & (1u << B));
+    lra_load_steps<NW, KS, B + 1>(T, addr, mask);
+  }
+}
 
 // Ring set-up shared by the gridder and the degridder: barriers, zeroed slab areas.
 template <int NW>
 __device__ __forceinline__ void lra_region_ring_init(const lra_region_args& a, unsigned char* smem,
                                                      uint32_t full0, uint32_t empty0) {
   if (threadIdx.x == 0) {
-    for (int s = 0; s < a.nslot; ++s) { lra_mbar_init(full0 + 8 * s, 1); lra_mbar_init(empty0 + 8 * s, NW); }
+    for (int s = 0; s < a.nslot; ++s) { lra_mbar_init(full0 + 8 * s, 1); lra_mbar_init(empty0 + 8 * s, NW * 32); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   const int area16 = (a.slot_bytes - LRA_SLOT_VAL) >> 4;   // everything behind the batch record

@@ -62,6 +62,8 @@ __global__ void __launch_bounds__(256) lra_work_kernel(const lra_work_args a) {
   __shared__ unsigned item_tile[LRA_CHUNK], item_first_run[LRA_CHUNK + 1], item_base[LRA_CHUNK], run_pos[LRA_CHUNK + 1];
   __shared__ unsigned short run_item[LRA_CHUNK];
   __shared__ unsigned char item_sup[LRA_CHUNK];
+  __shared__ lra_geom geom[LRA_NCLASS];   // per support class, once per block (lra_make_geom is not cheap)
+  if (threadIdx.x < LRA_NCLASS) geom[threadIdx.x] = lra_make_geom(2 * threadIdx.x + 1, a.tile_x, a.tile_y, a.ng);
   if (threadIdx.x < 2 * LRA_NCLASS) (&cls_cnt[0][0])[threadIdx.x] = 0;
   // ---- flags of the thread's 4 consecutive positions ----
   const long long i0 = lo + threadIdx.x * 4;
@@ -131,7 +133,7 @@ __global__ void __launch_bounds__(256) lra_work_kernel(const lra_work_args a) {
   for (unsigned j = threadIdx.x; j < n_items_blk; j += 256) {
     const unsigned S = item_sup[j], c = (unsigned)lra_class_of((int)S);
     const unsigned nruns = item_first_run[j + 1] - item_first_run[j];
-    const unsigned per = (unsigned)lra_make_geom((int)S, a.tile_x, a.tile_y, a.ng).per_batch;
+    const unsigned per = (unsigned)geom[c].per_batch;
     const unsigned nb = (nruns + per - 1) / per;
     if (!FILL) {
       atomicAdd(&cls_cnt[0][c], 1u);
@@ -155,7 +157,7 @@ __global__ void __launch_bounds__(256) lra_work_kernel(const lra_work_args a) {
   for (unsigned j = threadIdx.x; j < n_runs_blk; j += 256) {
     const unsigned it = run_item[j], S = item_sup[it], c = (unsigned)lra_class_of((int)S);
     const unsigned first_run = item_first_run[it], nruns = item_first_run[it + 1] - first_run;
-    const unsigned per = (unsigned)lra_make_geom((int)S, a.tile_x, a.tile_y, a.ng).per_batch;
+    const unsigned per = (unsigned)geom[c].per_batch;
     const unsigned q = j - first_run, b = q / per, r = q - b * per;
     uint32_t* rec16 = a.batch + (a.counters[LRA_CNT_BATCH_OFF + c] + item_base[it] + b) * 16ull;
     rec16[4 + r] = a.rec[run_pos[j]].y;
@@ -172,7 +174,7 @@ __global__ void __launch_bounds__(256) lra_work_kernel(const lra_work_args a) {
     const long long i = i0 + e;
     if (i < hi) {
       const unsigned j = my_run[e], it = run_item[j];
-      const lra_geom q = lra_make_geom((int)sp[e], a.tile_x, a.tile_y, a.ng);
+      const lra_geom& q = geom[lra_class_of((int)sp[e])];
       const unsigned r = (j - item_first_run[it]) % (unsigned)q.per_batch;
       const int ix = rc[e].x & 0xffff, iy = rc[e].x >> 16;
       const int ox = ix - ((ix >> a.shift_x) << a.shift_x), oy = iy - ((iy >> a.shift_y) << a.shift_y);
