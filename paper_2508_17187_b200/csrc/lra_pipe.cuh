@@ -85,12 +85,18 @@ __host__ __device__ inline lra_geom lra_make_geom(int S, int tile_x, int tile_y,
   q.span = (S - 1) * q.rx + S;
   const int chunks = (q.rx * q.ry + 63) / 64;
   q.nw = 0; q.ks = 0;
-  for (int nw = 1; nw <= 16; nw <<= 1) {
-    int ks = (chunks + nw - 1) / nw;
-    if (ks > lra_ks_max(ngp)) continue;
-    if ((ks & 1) && ks + 1 <= lra_ks_max(ngp) && ngp < 4) ++ks;
-    q.nw = nw; q.ks = ks;
-    break;
+#ifndef LRA_KS_PREF
+#define LRA_KS_PREF 8   // preferred steps per warp (measured on cfg3: 3, i.e. more and lighter warps, is 8 % slower: the per-point overhead of a warp dominates)
+#endif
+  for (int pass = 0; pass < 2 && q.nw == 0; ++pass) {
+    const int lim = pass == 0 ? (LRA_KS_PREF < lra_ks_max(ngp) ? LRA_KS_PREF : lra_ks_max(ngp)) : lra_ks_max(ngp);
+    for (int nw = 1; nw <= 16; nw <<= 1) {
+      int ks = (chunks + nw - 1) / nw;
+      if (ks > lim) continue;
+      if (pass == 1 && (ks & 1) && ks + 1 <= lim && ngp < 4) ++ks;
+      q.nw = nw; q.ks = ks;
+      break;
+    }
   }
   q.core = lra_slab_complex(S, tile_x);
   q.stride = q.core + LRA_GAP;
