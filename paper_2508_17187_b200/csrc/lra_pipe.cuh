@@ -89,11 +89,11 @@ __host__ __device__ inline lra_geom lra_make_geom(int S, int tile_x, int tile_y,
 #define LRA_KS_PREF 8   // preferred steps per warp (measured on cfg3: 3, i.e. more and lighter warps, is 8 % slower: the per-point overhead of a warp dominates)
 #endif
   for (int pass = 0; pass < 2 && q.nw == 0; ++pass) {
-    const int lim = pass == 0 ? (LRA_KS_PREF < lra_ks_max(ngp) ? LRA_KS_PREF : lra_ks_max(ngp)) : lra_ks_max(ngp);
+    const int lim = pass == 0 && LRA_KS_PREF < lra_ks_max(ngp) ? LRA_KS_PREF : lra_ks_max(ngp);
     for (int nw = 1; nw <= 16; nw <<= 1) {
       int ks = (chunks + nw - 1) / nw;
+      if (ks == 5 || ks == 7) ++ks;   // the kernels are instantiated for KS = 1, 2, 3, 4, 6, 8
       if (ks > lim) continue;
-      if (pass == 1 && (ks & 1) && ks + 1 <= lim && ngp < 4) ++ks;
       q.nw = nw; q.ks = ks;
       break;
     }
