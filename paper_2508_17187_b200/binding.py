@@ -80,14 +80,19 @@ def _check(rc: int, plan=None):
         raise LraError(f"liblra: {msg} [code {rc}]")
 
 
-def _dev(t, dtype=None) -> Optional[int]:
-    """Device pointer of a contiguous CUDA tensor (None passes NULL)."""
+_plan_device = {}   # plan handle -> CUDA device index (argument checks only)
+
+
+def _dev(t, dtype=None, plan=None) -> Optional[int]:
+    """Device pointer of a contiguous CUDA tensor on the plan's device (None passes NULL)."""
     if t is None:
         return None
     if not t.is_cuda or not t.is_contiguous():
         raise LraError("expected a contiguous CUDA tensor")
     if dtype is not None and t.dtype != dtype:
         raise LraError(f"expected dtype {dtype}, got {t.dtype}")
+    if plan is not None and plan in _plan_device and t.device.index != _plan_device[plan]:
+        raise LraError(f"tensor on cuda:{t.device.index}, plan on cuda:{_plan_device[plan]}")
     return t.data_ptr()
 
 
@@ -98,7 +103,8 @@ def _host(a: np.ndarray, dtype) -> np.ndarray:
 def lra_plan_create(nx, ny, ncorr, nterms, oversampling, scale_u, scale_v, cf_support, cf_offset, cf_data,
                     tile=0, sort_mode=LRA_SORT_TILE_CF, device=0, stream=None, tile_x=0) -> int:
     """-> opaque plan handle (int).  cf_* are HOST numpy arrays (lra.h: lra_plan_desc).  tile = 0: the library's
-    default 8 x 64 strips; tile_x = 0 with tile != 0: square tiles."""
+    default 8 x 8 tiles; tile_x = 0 with tile != 0: square tiles.  stream: a CUDA stream handle (int), 0 / None = the
+    default stream."""
     sup = _host(cf_support, np.int32)
     off = _host(cf_offset, np.int64)
     dat = _host(cf_data, np.complex64)
@@ -106,11 +112,13 @@ def lra_plan_create(nx, ny, ncorr, nterms, oversampling, scale_u, scale_v, cf_su
                       sup.ctypes.data, off.ctypes.data, dat.ctypes.data, device, stream or 0, tile_x)
     h = C.c_void_p()
     _check(lib().lra_plan_create(C.byref(h), C.byref(d)))
+    _plan_device[h.value] = int(device)
     return h.value
 
 
 def lra_plan_destroy(plan: int):
     _check(lib().lra_plan_destroy(plan))
+    _plan_device.pop(plan, None)
 
 
 def lra_bin(plan: int, uvw_m, freq_hz, cf_index=None):
@@ -118,7 +126,12 @@ def lra_bin(plan: int, uvw_m, freq_hz, cf_index=None):
     import torch
     f = _host(freq_hz, np.float64)
     nrow, nchan = int(uvw_m.shape[0]), len(f)
-    _check(lib().lra_bin(plan, nrow, nchan, _dev(uvw_m, torch.float64), f.ctypes.data, _dev(cf_index, torch.int32)), plan)
+    if tuple(uvw_m.shape) != (nrow, 3):
+        raise LraError(f"uvw_m must be [nrow, 3], got {tuple(uvw_m.shape)}")
+    if cf_index is not None and tuple(cf_index.shape) != (nrow, nchan):
+        raise LraError(f"cf_index must be [nrow, nchan] = {(nrow, nchan)}, got {tuple(cf_index.shape)}")
+    _check(lib().lra_bin(plan, nrow, nchan, _dev(uvw_m, torch.float64, plan), f.ctypes.data,
+                         _dev(cf_index, torch.int32, plan)), plan)
 
 
 def lra_bin_export(plan: int, ix=None, iy=None, fx=None, fy=None, key=None, perm=None, tile_start=None) -> int:
@@ -131,14 +144,14 @@ def lra_bin_export(plan: int, ix=None, iy=None, fx=None, fy=None, key=None, perm
 
 def lra_grid(plan: int, vis, wt, tau, grid, sumwt=None):
     import torch
-    _check(lib().lra_grid(plan, _dev(vis, torch.complex64), _dev(wt, torch.float32), _dev(tau, torch.float32),
-                          _dev(grid, torch.complex64), _dev(sumwt, torch.float64)), plan)
+    _check(lib().lra_grid(plan, _dev(vis, torch.complex64, plan), _dev(wt, torch.float32, plan), _dev(tau, torch.float32, plan),
+                          _dev(grid, torch.complex64, plan), _dev(sumwt, torch.float64, plan)), plan)
 
 
 def lra_degrid(plan: int, grid, tau, vis_in, vis_out):
     import torch
-    _check(lib().lra_degrid(plan, _dev(grid, torch.complex64), _dev(tau, torch.float32), _dev(vis_in, torch.complex64),
-                            _dev(vis_out, torch.complex64)), plan)
+    _check(lib().lra_degrid(plan, _dev(grid, torch.complex64, plan), _dev(tau, torch.float32, plan),
+                            _dev(vis_in, torch.complex64, plan), _dev(vis_out, torch.complex64, plan)), plan)
 
 
 def lra_launch_count(plan: int) -> int:
