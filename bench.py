@@ -9,7 +9,10 @@ supports 9..65, oversampling 8).  With N > 1 ranks every rank runs the same-size
 seeded per rank) and the per-rank grids are summed with one NCCL all-reduce per step (accumulation of partial
 grids, PAPER.md:347).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3] [--small]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1..5] [--small]
+
+`--gpus N` with N > 1 starts N ranks itself (torch.distributed.run on 127.0.0.1) unless it already runs under
+torchrun; the other BASELINE.json configurations are `--config 1`, `2`, `4`, `5` (one line each, same script).
 """
 from __future__ import annotations
 
@@ -30,7 +33,7 @@ sys.path.insert(0, ROOT)
 from paper_2508_17187_b200 import workloads as W  # noqa: E402
 
 FP32_PEAK_TFLOPS_NOMINAL = 148 * 128 * 2 * 1.965e9 / 1e12   # 148 SMs x 128 FP32 lanes x 2 flop x 1965 MHz
-NCU_DRAM_BYTES_GRID_CFG3 = 4.313e9   # measured once under ncu, see profiles/r1_c_summary.md ("DRAM and L2 traffic")
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r2_traffic.json")   # written from the ncu capture (profiles/r2_traffic.md)
 METRIC = "visibility points per second through bin+grid+degrid"
 UNIT = "vis_points/s"
 
@@ -49,6 +52,30 @@ def parse():
     ap.add_argument("--tile", type=int, default=0, help="uv-tile height (0 = the config's, i.e. the library default)")
     ap.add_argument("--tile-x", type=int, default=0, help="uv-tile width (with --tile)")
     return ap.parse_args()
+
+
+def source_hash():
+    """sha256 over the CUDA sources: ties a stored ncu measurement to the code it was taken on (no .git on the GPU box)."""
+    import glob
+    import hashlib
+    h = hashlib.sha256()
+    for f in sorted(glob.glob(os.path.join(ROOT, "paper_2508_17187_b200", "csrc", "*.cu*"))):
+        h.update(os.path.basename(f).encode())
+        h.update(open(f, "rb").read())
+    return h.hexdigest()[:16]
+
+
+def stored_traffic(cfg_name):
+    """DRAM bytes per lra_grid call from the committed ncu capture, or None when the sources have changed since."""
+    try:
+        t = json.load(open(TRAFFIC_FILE))
+    except Exception:
+        return None, "no profiles/r2_traffic.json"
+    if t.get("workload") != cfg_name:
+        return None, f"profiles/r2_traffic.json is for {t.get('workload')}"
+    if t.get("source_hash") != source_hash():
+        return None, "profiles/r2_traffic.json was captured on other sources (hash differs): not reported"
+    return t, t.get("how", "")
 
 
 def measured_peaks():
@@ -113,32 +140,41 @@ def make_workload(args, rank):
     return wl
 
 
-def oracle_sample(wl, args, target_taps=6.0e9):
-    """The oracle as it stands (oracle/lra_ref.c, fp64, OpenMP row bands) on a bounded sample of the workload:
-    the first `nt` time samples (all baselines, channels, correlations), bin + grid + degrid.  Returns
-    (points/s, seconds, cores, sample description, grid taps/s)."""
+def oracle_sample(wl, args, target_taps=6.0e9, nthreads=0):
+    """The oracle as it stands (oracle/lra_ref.c, fp64, OpenMP row bands) on a bounded sample of the workload: every
+    k-th time sample (a uniform stride over the whole track, so the sample has the workload's w distribution; all
+    baselines, channels, correlations), bin + grid + degrid.  Returns (points/s, seconds, threads, sample description,
+    grid taps/s)."""
     from oracle import lra_ref as R
     cfg = wl.cfg
     per_time = max(1, wl.sum_s2() * cfg.ncorr * cfg.nterms // cfg.ntimes)          # grid taps per time sample
     nt = int(max(1, min(cfg.ntimes, target_taps // (2 * per_time))))               # grid + degrid
-    rows = W.N_BL * nt if cfg.kind != "disk" else cfg.nrow
-    sl = slice(0, rows)
-    cfi = None if wl.cf_index is None else wl.cf_index[sl]
+    if cfg.kind != "disk":
+        stride = max(1, cfg.ntimes // nt)
+        times = np.arange(0, cfg.ntimes, stride)[:nt]
+        rows = (times[:, None] * W.N_BL + np.arange(W.N_BL)[None, :]).ravel()      # rows are time-major, baseline-minor
+        what = f"every {stride}-th of {cfg.ntimes} time samples ({len(times)} samples)"
+    else:
+        rows = np.arange(cfg.nrow)
+        what = "all rows"
+    uvw, vis, wt = wl.uvw[rows], wl.vis[rows], wl.wt[rows]
+    cfi = None if wl.cf_index is None else wl.cf_index[rows]
     plan = R.plan_for(wl, sort_mode=R.SORT_TILE_CF)
-    cores = R.max_threads()
+    threads = nthreads or R.max_threads()
     t0 = time.perf_counter()
-    plan.bin(wl.uvw[sl], wl.freq, cfi)
+    plan.bin(uvw, wl.freq, cfi)
     t1 = time.perf_counter()
-    grid, _ = plan.grid(wl.uvw[sl], wl.freq, cfi, wl.vis[sl], wl.wt[sl], wl.tau)
+    grid, _ = plan.grid(uvw, wl.freq, cfi, vis, wt, wl.tau, nthreads=threads)
     t2 = time.perf_counter()
-    plan.degrid(wl.uvw[sl], wl.freq, cfi, grid, wl.tau, vis_in=wl.vis[sl])
+    plan.degrid(uvw, wl.freq, cfi, grid, wl.tau, vis_in=vis, nthreads=threads)
     t3 = time.perf_counter()
-    npts = rows * cfg.nchan
-    taps = (wl.sum_s2() if cfi is None else int((np.bincount(cfi.ravel(), minlength=len(wl.cf.support)).astype(np.int64)
-                                                 * wl.cf.support.astype(np.int64) ** 2).sum())) * cfg.ncorr * cfg.nterms
-    desc = (f"first {nt} of {cfg.ntimes} time samples ({npts} points x {cfg.ncorr} corr), bin {t1 - t0:.2f}s + grid "
-            f"{t2 - t1:.2f}s + degrid {t3 - t2:.2f}s, fp64, {cores} OpenMP threads")
-    return npts / (t3 - t0), t3 - t0, cores, desc, taps / (t2 - t1)
+    npts = len(rows) * cfg.nchan
+    taps = (npts * int(wl.cf.support[0]) ** 2 if cfi is None else
+            int((np.bincount(cfi.ravel(), minlength=len(wl.cf.support)).astype(np.int64)
+                 * wl.cf.support.astype(np.int64) ** 2).sum())) * cfg.ncorr * cfg.nterms
+    desc = (f"{what}, {npts} points x {cfg.ncorr} corr: bin {t1 - t0:.2f}s (1 thread) + grid {t2 - t1:.2f}s + degrid "
+            f"{t3 - t2:.2f}s, fp64, {threads} OpenMP thread(s) of {os.cpu_count()} hardware threads")
+    return npts / (t3 - t0), t3 - t0, threads, desc, taps / (t2 - t1)
 
 
 def run_reference(args):
@@ -337,13 +373,14 @@ def run_ours(args):
                         "1965 MHz = %.2f; MEASURED_PEAKS.json has no FP32 entry" % FP32_PEAK_TFLOPS_NOMINAL)
         except Exception:
             fma_peak, peak_src = FP32_PEAK_TFLOPS_NOMINAL, "derived: 148 SM x 128 FP32 lanes x 2 flop x 1965 MHz"
+        traffic, traffic_src = (None, "not the default launch configuration") if (args.small or args.tile) else stored_traffic(cfg.name)
         roofline = {"bound": "alu", "kernel": "lra_grid_region_kernel (all per-support-class launches of one lra_grid call, "
                                               "CUDA events on the plan's stream around the call)",
                     "achieved": achieved, "peak": fma_peak, "unit": "TFLOP/s", "frac": achieved / fma_peak,
                     "peak_source": peak_src,
-                    "traffic": NCU_DRAM_BYTES_GRID_CFG3 if (cfg.cfg_id == 3 and not args.small and not args.tile) else None,
-                    "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum over the 29 lra_grid_region_kernel launches of one "
-                                      "lra_grid call, profiles/r1_c_summary.md (ncu, cfg3); algorithmic bytes 2.37e9",
+                    "traffic": None if not traffic else traffic.get("region_kernels_dram_bytes"),
+                    "traffic_call": None if not traffic else traffic.get("lra_grid_call_dram_bytes"),
+                    "traffic_source": traffic_src, "algorithmic_bytes": 2.37e9 if cfg.cfg_id == 3 and not args.small else None,
                     "tap_updates_per_launch": grid_taps, "tap_updates_per_s": grid_taps / (med["grid"] * 1e-3),
                     "degrid_frac": (grid_flops / (med["degrid"] * 1e-3) / 1e12 / fma_peak) if med["degrid"] else None,
                     "degrid_tap_updates_per_s": grid_taps / (med["degrid"] * 1e-3) if med["degrid"] else None,
@@ -361,17 +398,38 @@ def run_ours(args):
             line["e2e"] = e2e
         if not args.no_cpu_baseline and world == 1:
             v, secs, cores, desc, gt = oracle_sample(wl, args)
+            v1, secs1, _, desc1, gt1 = oracle_sample(wl, args, target_taps=4.0e8, nthreads=1)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
-                                    "grid_tap_updates_per_s": gt}
+                                    "grid_tap_updates_per_s": gt, "hardware_threads": os.cpu_count(),
+                                    "single_thread": {"value": v1, "unit": UNIT, "cores": 1, "sample": desc1,
+                                                      "grid_tap_updates_per_s": gt1}}
         print(json.dumps(line))
     B.lra_plan_destroy(plan)
     if world > 1:
         dist.destroy_process_group()
 
 
+def spawn_ranks(args):
+    """`python bench.py --gpus N` outside torchrun: start the N ranks ourselves (one process per GPU, NCCL over
+    NVLink), exactly as the driver's torchrun line would; NCCL's own init lines stay on stderr."""
+    import socket
+    import torch
+    have = torch.cuda.device_count()
+    if have < args.gpus:
+        raise SystemExit(f"bench.py --gpus {args.gpus}: only {have} CUDA device(s) visible")
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
+
+
 if __name__ == "__main__":
     a = parse()
     if a.impl == "reference":
         run_reference(a)
+    elif a.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        spawn_ranks(a)
     else:
         run_ours(a)
