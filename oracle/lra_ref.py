@@ -16,15 +16,16 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "liblra_ref.so")
 _SRC = os.path.join(_HERE, "lra_ref.c")
+_SRCS = [_SRC, os.path.join(_HERE, "lra_ref_image.c")]
 
 SORT_TILE, SORT_TILE_CF = 0, 1
 
 
 def build(force: bool = False) -> str:
     """gcc -O2 -ffp-contract=off -fopenmp: no FMA contraction, so each * and + rounds once (R2)."""
-    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < max(os.path.getmtime(f) for f in _SRCS):
         subprocess.check_call(["gcc", "-O2", "-std=c99", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared",
-                               "-o", _SO, _SRC, "-lm"])
+                               "-o", _SO] + _SRCS + ["-lm"])
     return _SO
 
 
@@ -153,3 +154,30 @@ def plan_for(wl, nterms=None, sort_mode=SORT_TILE, tile=None, tile_x=0) -> RefPl
     return RefPlan(c.nx, c.ny, c.ncorr, c.nterms if nterms is None else nterms, c.oversampling, wl.scale_u,
                    wl.scale_v, wl.cf.support, wl.cf.offset, wl.cf.data, tile=tile, sort_mode=sort_mode,
                    tile_x=tile_x)
+
+
+def image(grid, sumwt=None, corr_x=None, corr_y=None) -> np.ndarray:
+    """lra_ref_image: grid [..., ny, nx] complex -> real image of the same leading shape (oracle/lra_ref_image.c)."""
+    grid = np.ascontiguousarray(grid, dtype=np.complex128)
+    ny, nx = grid.shape[-2:]
+    ng = int(np.prod(grid.shape[:-2], dtype=np.int64)) if grid.ndim > 2 else 1
+    sumwt = None if sumwt is None else np.ascontiguousarray(sumwt, dtype=np.float64).reshape(ng)
+    corr_x = None if corr_x is None else np.ascontiguousarray(corr_x, dtype=np.float64)
+    corr_y = None if corr_y is None else np.ascontiguousarray(corr_y, dtype=np.float64)
+    out = np.empty(grid.shape, dtype=np.float64)
+    rc = lib().lra_ref_image(C.c_int32(ng), C.c_int32(ny), C.c_int32(nx), _p(grid), _p(sumwt), _p(corr_x), _p(corr_y), _p(out))
+    assert rc == 0
+    return out
+
+
+def model_grid(img, corr_x=None, corr_y=None) -> np.ndarray:
+    """lra_ref_model_grid: real image [..., ny, nx] -> complex grid of the same shape (oracle/lra_ref_image.c)."""
+    img = np.ascontiguousarray(img, dtype=np.float64)
+    ny, nx = img.shape[-2:]
+    ng = int(np.prod(img.shape[:-2], dtype=np.int64)) if img.ndim > 2 else 1
+    corr_x = None if corr_x is None else np.ascontiguousarray(corr_x, dtype=np.float64)
+    corr_y = None if corr_y is None else np.ascontiguousarray(corr_y, dtype=np.float64)
+    out = np.empty(img.shape, dtype=np.complex128)
+    rc = lib().lra_ref_model_grid(C.c_int32(ng), C.c_int32(ny), C.c_int32(nx), _p(img), _p(corr_x), _p(corr_y), _p(out))
+    assert rc == 0
+    return out

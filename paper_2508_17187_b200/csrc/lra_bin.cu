@@ -242,7 +242,7 @@ int lra_bin_impl(lra_plan* p, int64_t nrow, int32_t nchan, const double* uvw, co
   }
   LRA_CUDA(p, cudaMemcpyAsync(p->d_su, su.data(), nchan * sizeof(double), cudaMemcpyHostToDevice, p->stream));
   LRA_CUDA(p, cudaMemcpyAsync(p->d_sv, sv.data(), nchan * sizeof(double), cudaMemcpyHostToDevice, p->stream));
-  LRA_CUDA(p, cudaStreamSynchronize(p->stream));  // su / sv are stack-owned
+  // (pageable source: the runtime stages the bytes before cudaMemcpyAsync returns, so su / sv may go out of scope)
   LRA_CUDA(p, cudaMemsetAsync(p->counters, 0, LRA_TICKET0 * sizeof(unsigned long long), p->stream));
 
   unsigned long long per_tile = 1;

@@ -12,6 +12,7 @@ struct lra_work_args {
   uint4* work;
   uint32_t* batch;     // 16 words per batch
   uint4* pw;           // one 16-byte record per sorted position: {word, k, S, c_lo | c_hi << 16}
+  unsigned item_off[LRA_NCLASS], batch_off[LRA_NCLASS];   // FILL pass: first item / batch of every class (from the host)
 };
 
 // exclusive prefix sum over the block (256 threads); returns the block total through `total`
@@ -140,7 +141,7 @@ __global__ void __launch_bounds__(256) lra_work_kernel(const lra_work_args a) {
       atomicAdd(&cls_cnt[1][c], nb);
     } else {
       const unsigned base = (unsigned)atomicAdd(&a.counters[LRA_CNT_BATCH_CUR + c], (unsigned long long)nb);
-      const unsigned long long idx = a.counters[LRA_CNT_ITEM_OFF + c] + atomicAdd(&a.counters[LRA_CNT_ITEM_CUR + c], 1ull);
+      const unsigned long long idx = a.item_off[c] + atomicAdd(&a.counters[LRA_CNT_ITEM_CUR + c], 1ull);
       a.work[idx] = make_uint4(item_tile[j], base, nb, S);
       item_base[j] = base;
     }
@@ -159,7 +160,7 @@ __global__ void __launch_bounds__(256) lra_work_kernel(const lra_work_args a) {
     const unsigned first_run = item_first_run[it], nruns = item_first_run[it + 1] - first_run;
     const unsigned per = (unsigned)geom[c].per_batch;
     const unsigned q = j - first_run, b = q / per, r = q - b * per;
-    uint32_t* rec16 = a.batch + (a.counters[LRA_CNT_BATCH_OFF + c] + item_base[it] + b) * 16ull;
+    uint32_t* rec16 = a.batch + ((unsigned long long)a.batch_off[c] + item_base[it] + b) * 16ull;
     rec16[4 + r] = a.rec[run_pos[j]].y;
     if (r == 0) {
       const unsigned nr = nruns - b * per < per ? nruns - b * per : per;
@@ -202,6 +203,7 @@ int lra_build_work(lra_plan* p) {
   lra_work_args a;
   a.rec = p->rec; a.counters = p->counters; a.ntx = p->ntx; a.tile_x = p->tile_x; a.tile_y = p->tile; a.ng = p->ncorr * p->nterms;
   a.work = nullptr; a.batch = nullptr; a.pw = nullptr;
+  for (int c = 0; c < LRA_NCLASS; ++c) a.item_off[c] = a.batch_off[c] = 0;
   a.shift_x = a.shift_y = 0;
   while ((1 << a.shift_x) < p->tile_x) ++a.shift_x;
   while ((1 << a.shift_y) < p->tile) ++a.shift_y;
@@ -211,18 +213,17 @@ int lra_build_work(lra_plan* p) {
   lra_work_kernel<false><<<blocks, 256, 0, p->stream>>>(a);
   LRA_LAUNCH_CHECK(p);
   static_assert(LRA_CNT_BATCHES == LRA_CNT_ITEMS + 128 && LRA_CNT_BATCH_OFF == LRA_CNT_ITEM_OFF + 128, "counter layout");
-  unsigned long long h[256], off[256];
+  unsigned long long h[256];
   LRA_CUDA(p, cudaMemcpyAsync(h, p->counters + LRA_CNT_ITEMS, sizeof h, cudaMemcpyDeviceToHost, p->stream));
-  LRA_CUDA(p, cudaStreamSynchronize(p->stream));
+  LRA_CUDA(p, cudaStreamSynchronize(p->stream));   // the one host synchronisation of lra_bin: the list sizes
   int64_t items = 0, batches = 0;
-  for (int c = 0; c < 128; ++c) off[c] = off[128 + c] = 0;
   for (int c = 0; c < LRA_NCLASS; ++c) {
     p->n_items[c] = (int64_t)h[c];
     p->n_batches[c] = (int64_t)h[128 + c];
     p->item_off[c] = items;
     p->batch_off[c] = batches;
-    off[c] = (unsigned long long)items;
-    off[128 + c] = (unsigned long long)batches;
+    a.item_off[c] = (unsigned)items;
+    a.batch_off[c] = (unsigned)batches;
     items += p->n_items[c];
     batches += p->n_batches[c];
   }
@@ -231,10 +232,8 @@ int lra_build_work(lra_plan* p) {
   if ((rc = lra_grow(p, &p->batch, &bwords, batches * 16))) return rc;
   p->batch_capacity = bwords / 16;
   if ((rc = lra_grow(p, &p->pw, &p->pw_capacity, n))) return rc;
-  LRA_CUDA(p, cudaMemcpyAsync(p->counters + LRA_CNT_ITEM_OFF, off, sizeof off, cudaMemcpyHostToDevice, p->stream));
   a.work = p->work; a.batch = p->batch; a.pw = p->pw;
   lra_work_kernel<true><<<blocks, 256, 0, p->stream>>>(a);
   LRA_LAUNCH_CHECK(p);
-  LRA_CUDA(p, cudaStreamSynchronize(p->stream));  // `off` is stack-owned
   return LRA_OK;
 }
