@@ -82,6 +82,8 @@ int lra_plan_destroy(lra_plan* p);
  *   freq_hz     : HOST double [nchan]  (small; the per-channel scale (freq/c)*scale is formed on the host)
  *   cf_index    : device int32 [nrow][nchan] kernel of every point, or NULL (=> kernel 0)
  * The input arrays are not referenced after the call's stream work completes.
+ * Synchronises the plan's stream ONCE, between its two passes over the sorted points (the host sizes the work lists of
+ * lra_grid / lra_degrid from the per-class counts), and again whenever the plan's arrays have to grow.
  * Errors: LRA_EINVAL, LRA_ENOMEM (growing the plan's bin arrays), LRA_ECUDA. */
 int lra_bin(lra_plan* p, int64_t nrow, int32_t nchan, const double* uvw_m, const double* freq_hz,
             const int32_t* cf_index);
@@ -115,6 +117,26 @@ int lra_grid(lra_plan* p, const void* vis_c64, const float* wt, const float* tau
  *                (vis_out may alias vis_in)
  * Errors: LRA_ESTATE before lra_bin, LRA_EINVAL, LRA_ECUDA. */
 int lra_degrid(lra_plan* p, const void* grid_c64, const float* tau, const void* vis_in_c64, void* vis_out_c64);
+
+/* The transforms either side of the path (Eq. 23: I^R = F^dagger G W [...];
+ * PAPER.md:346 "UpdateDir"), readings R17-R19 of DESIGN.md.  nx and ny must be even.
+ *
+ * lra_image: the residual / dirty image of the gridded data,
+ *   image[t][p][m][l] = Re( sum_{y,x} grid[t][p][y][x] e^{+2 pi i ((x-nx/2)(l-nx/2)/nx + (y-ny/2)(m-ny/2)/ny)} )
+ *                       * corr_x[l] * corr_y[m] / sumwt[t][p]
+ * (centred inverse DFT without 1/N, the image-plane correction for the gridding taper as a separable factor, and the
+ * sum-of-weights normalisation).  cuFFT C2C does the transform; the sign / correction / normalisation kernels are the
+ * library's own.
+ *   grid_c64 : device complex64 [nterms][ncorr][ny][nx], read only
+ *   sumwt    : device double [nterms][ncorr] or NULL (=> 1);  corr_x: device float [nx] or NULL (=> 1);  corr_y: [ny]
+ *   image    : device float [nterms][ncorr][ny][nx], overwritten
+ * lra_model_grid: the forward transform of a model image onto the uv grid (the "F I^M" that lra_degrid reads),
+ *   grid[t][p][y][x] = sum_{m,l} image[t][p][m][l] corr_x[l] corr_y[m] e^{-2 pi i (...)}      (grid overwritten).
+ * The plan keeps a complex scratch grid and the cuFFT plan (allocated on first use).
+ * Errors: LRA_EINVAL (odd nx / ny, NULL grid / image), LRA_ENOMEM, LRA_ECUDA (also any cuFFT failure). */
+int lra_image(lra_plan* p, const void* grid_c64, const double* sumwt, const float* corr_x, const float* corr_y,
+              float* image);
+int lra_model_grid(lra_plan* p, const float* image, const float* corr_x, const float* corr_y, void* grid_c64);
 
 /* Number of kernel launches the plan has enqueued since creation (for bench.py's gpu_launches). */
 int64_t lra_launch_count(const lra_plan* p);

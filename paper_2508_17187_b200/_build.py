@@ -54,8 +54,9 @@ def build(force: bool = False, verbose: bool = False, defines=()) -> str:
         for out in ex.map(compile_one, SOURCES):
             if out:
                 print(out)
+    cuda_lib = os.path.join(os.path.dirname(os.path.dirname(os.path.realpath(nvcc))), "lib64")
     subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-cudart", "static",
-                           "-o", SO_PATH] + [_obj(s) for s in SOURCES])
+                           "-o", SO_PATH] + [_obj(s) for s in SOURCES] + ["-lcufft", "-Xlinker", f"-rpath={cuda_lib}"])
     return SO_PATH
 
 

@@ -51,6 +51,8 @@ def lib() -> C.CDLL:
         L.lra_bin_export.argtypes = [vp] * 8 + [C.POINTER(i64)]
         L.lra_grid.argtypes = [vp] * 6
         L.lra_degrid.argtypes = [vp] * 5
+        L.lra_image.argtypes = [vp] * 6
+        L.lra_model_grid.argtypes = [vp] * 5
         L.lra_launch_count.argtypes = [vp]
         L.lra_launch_count.restype = i64
         L.lra_tap_count.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
@@ -65,7 +67,8 @@ def lib() -> C.CDLL:
     return _lib
 
 
-EXPORTED = ["lra_plan_create", "lra_plan_destroy", "lra_bin", "lra_bin_export", "lra_grid", "lra_degrid",
+EXPORTED = ["lra_plan_create", "lra_plan_destroy", "lra_bin", "lra_bin_export", "lra_grid", "lra_degrid", "lra_image",
+            "lra_model_grid",
             "lra_launch_count", "lra_tap_count", "lra_set_variant", "lra_strerror", "lra_last_cuda_error",
             "lra_diag_fma_tflops", "lra_diag_l2_gbs"]
 
@@ -152,6 +155,21 @@ def lra_degrid(plan: int, grid, tau, vis_in, vis_out):
     import torch
     _check(lib().lra_degrid(plan, _dev(grid, torch.complex64, plan), _dev(tau, torch.float32, plan),
                             _dev(vis_in, torch.complex64, plan), _dev(vis_out, torch.complex64, plan)), plan)
+
+
+def lra_image(plan: int, grid, sumwt, corr_x, corr_y, image):
+    """grid complex64 [nterms, ncorr, ny, nx] -> image float32 of the same shape (lra.h: lra_image)."""
+    import torch
+    _check(lib().lra_image(plan, _dev(grid, torch.complex64, plan), _dev(sumwt, torch.float64, plan),
+                           _dev(corr_x, torch.float32, plan), _dev(corr_y, torch.float32, plan),
+                           _dev(image, torch.float32, plan)), plan)
+
+
+def lra_model_grid(plan: int, image, corr_x, corr_y, grid):
+    """image float32 [nterms, ncorr, ny, nx] -> grid complex64 of the same shape (lra.h: lra_model_grid)."""
+    import torch
+    _check(lib().lra_model_grid(plan, _dev(image, torch.float32, plan), _dev(corr_x, torch.float32, plan),
+                                _dev(corr_y, torch.float32, plan), _dev(grid, torch.complex64, plan)), plan)
 
 
 def lra_launch_count(plan: int) -> int:

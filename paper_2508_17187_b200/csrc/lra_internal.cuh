@@ -69,6 +69,10 @@ struct lra_plan {
   int64_t n_batches[LRA_NCLASS], batch_off[LRA_NCLASS];  // batches per class, first batch of the class in `batch`
   cudaStream_t aux[LRA_NAUX];          // per-class launches run concurrently on these, forked from / joined to `stream`
   cudaEvent_t ev_fork, ev_join[LRA_NAUX];
+  // ---- image-plane transforms (lra_image.cu) ----
+  float2* fft_work;         // complex scratch [nterms*ncorr][ny][nx]
+  int fft_plan;             // cufftHandle (0 = none yet)
+  bool fft_ready;
   // ---- misc ----
   int32_t grid_variant, degrid_variant;
   int64_t launches;

@@ -126,10 +126,13 @@ extern "C" int lra_plan_create(lra_plan** out, const lra_plan_desc* d) {
   return LRA_OK;
 }
 
+void lra_fft_release(lra_plan* p);   // lra_image.cu
+
 extern "C" int lra_plan_destroy(lra_plan* p) {
   if (!p) return LRA_EINVAL;
   cudaSetDevice(p->device);
   cudaStreamSynchronize(p->stream);
+  lra_fft_release(p);
   void* ptrs[] = {p->slabs, p->d_cf_support, p->d_slab_off, p->ix, p->iy, p->fx, p->fy, p->key, p->skey[0], p->skey[1],
                   p->sval[0], p->sval[1], p->hist, p->tile_start, p->rec, p->urec, p->counters, p->d_su, p->d_sv, p->work, p->batch, p->pw, p->prep};
   for (void* q : ptrs)

@@ -476,3 +476,70 @@ def test_repeated_calls_keep_parity(B, ref):
             assert_close(run.degrid(model, wl.tau, vis_in=wl.vis), want_v, f"degrid, repetition {it}")
     finally:
         run.close()
+
+
+# ---------------------------------------------------------------------------------------------------
+# NEXT-1: grid -> image (F^dagger, taper correction, sum-of-weights normalisation) and image -> grid (F)
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("ny,nx,ncorr,nterms", [(64, 64, 1, 1), (96, 128, 2, 2), (254, 130, 2, 1)])
+def test_image_and_model_grid(B, ref, ny, nx, ncorr, nterms):
+    """Both transforms against the oracle's centred DFT (relative L2 <= 1e-5, max abs <= 1e-4 max|.|): sizes with
+    nx/2 + ny/2 even and odd (the sign of the centring), non-square, several grids, with and without the factors."""
+    rng = np.random.default_rng(nx + ny)
+    sup, off, data = np.array([3], np.int32), np.array([0], np.int64), np.ones(9, np.complex64)
+    plan = B.lra_plan_create(nx, ny, ncorr, nterms, 1, 1.0, 1.0, sup, off, data)
+    try:
+        g = (rng.standard_normal((nterms, ncorr, ny, nx)) + 1j * rng.standard_normal((nterms, ncorr, ny, nx))).astype(np.complex64)
+        sw = rng.uniform(0.5, 3.0, (nterms, ncorr))
+        cx, cy = rng.uniform(0.5, 2.0, nx).astype(np.float32), rng.uniform(0.5, 2.0, ny).astype(np.float32)
+        img = torch.empty((nterms, ncorr, ny, nx), dtype=torch.float32, device="cuda")
+        for use in (True, False):
+            B.lra_image(plan, dev(g), dev(sw) if use else None, dev(cx) if use else None, dev(cy) if use else None, img)
+            torch.cuda.synchronize()
+            want = ref.image(g, sw if use else None, cx if use else None, cy if use else None)
+            got = img.cpu().numpy().astype(np.float64)
+            assert np.linalg.norm(got - want) <= 1e-5 * np.linalg.norm(want)
+            assert np.abs(got - want).max() <= 1e-4 * np.abs(want).max()
+        im = rng.standard_normal((nterms, ncorr, ny, nx)).astype(np.float32)
+        out = torch.empty((nterms, ncorr, ny, nx), dtype=torch.complex64, device="cuda")
+        B.lra_model_grid(plan, dev(im), dev(cx), dev(cy), out)
+        torch.cuda.synchronize()
+        assert_close(out.cpu().numpy(), ref.model_grid(im, cx, cy), "model grid")
+    finally:
+        B.lra_plan_destroy(plan)
+
+
+def test_major_cycle_on_device(B, ref):
+    """The whole UpdateDir of Eq. 23 on the device for cfg5-small: model image -> F -> degrid with fused residual ->
+    grid (two Taylor terms) -> F^dagger with normalisation, against the same chain through the oracle."""
+    wl = W.make_workload(W.small_config(5))
+    c = wl.cfg
+    rng = np.random.default_rng(55)
+    model_img = np.zeros((1, c.ncorr, c.ny, c.nx), np.float32)
+    for _ in range(20):
+        y, x = rng.integers(c.ny // 10, c.ny - c.ny // 10), rng.integers(c.nx // 10, c.nx - c.nx // 10)
+        model_img[0, :, y, x] = rng.uniform(0.1, 1.0)
+    rp1, rp2 = ref_for(ref, wl, nterms=1), ref_for(ref, wl, nterms=2)
+    mg = ref.model_grid(model_img).astype(np.complex64)                      # oracle chain
+    res_want = rp1.degrid(wl.uvw, wl.freq, wl.cf_index, mg.astype(np.complex128), None, vis_in=wl.vis)
+    g_want, sw_want = rp2.grid(wl.uvw, wl.freq, wl.cf_index, res_want.astype(np.complex64), wl.wt, wl.tau)
+    img_want = ref.image(g_want.astype(np.complex64), sw_want)
+    run1, run2 = run_for(B, wl, nterms=1), run_for(B, wl, nterms=2)
+    try:
+        d_mg = torch.empty((1, c.ncorr, c.ny, c.nx), dtype=torch.complex64, device="cuda")
+        B.lra_model_grid(run1.plan, dev(model_img), None, None, d_mg)
+        assert_close(d_mg.cpu().numpy(), mg, "model grid of the cycle")
+        res = torch.empty((c.nrow, c.nchan, c.ncorr), dtype=torch.complex64, device="cuda")
+        B.lra_degrid(run1.plan, d_mg, None, dev(wl.vis), res)
+        g = torch.zeros((2, c.ncorr, c.ny, c.nx), dtype=torch.complex64, device="cuda")
+        sw = torch.zeros((2, c.ncorr), dtype=torch.float64, device="cuda")
+        B.lra_grid(run2.plan, res, dev(wl.wt), dev(wl.tau), g, sw)
+        img = torch.empty((2, c.ncorr, c.ny, c.nx), dtype=torch.float32, device="cuda")
+        B.lra_image(run2.plan, g, sw, None, None, img)
+        torch.cuda.synchronize()
+        got = img.cpu().numpy().astype(np.float64)
+        assert np.linalg.norm(got - img_want) <= 1e-5 * np.linalg.norm(img_want) * 3      # three chained fp32 stages
+        assert np.abs(got - img_want).max() <= 1e-4 * np.abs(img_want).max()
+    finally:
+        run1.close()
+        run2.close()
