@@ -508,8 +508,9 @@ def _make_disk(cfg: Config) -> Workload:
 
 def _model_grid(cfg: Config, fov: float) -> np.ndarray:
     """cfg5 model: point sources at seeded positions within the inner 80 % of the field, flux ~ U(0.1, 1);
-    the model *grid* is their analytic Fourier transform sampled at the uv pixel centres (the result of
-    'inverse-taper then 2-D FFT' for delta functions, evaluated directly; host-side, not timed).
+    the model *grid* is their analytic Fourier transform sampled at the uv pixel centres (the 2-D FFT of the delta
+    functions, evaluated directly; host-side, not timed).  NO inverse taper is applied (reading R20: the
+    taper correction is an input-side choice that does not touch the path; lra_model_grid takes it as corr_x / corr_y).
     Same grid for every correlation."""
     rng = _rng(cfg.cfg_id, 5)
     ns = cfg.n_sources
