@@ -14,12 +14,12 @@ int lra_degrid_launch_ng(lra_plan* p, const lra_region_args& a, const lra_geom& 
 __global__ void __launch_bounds__(256)
 lra_degrid_finish_kernel(const uint4* __restrict__ pw, const unsigned long long* __restrict__ counters,
                          const float2* __restrict__ res, const float* __restrict__ tau, const float2* vis_in,
-                         float2* vis_out, int nchan, int ncorr, int nterms, long long npoints, lra_fallback_mask fb) {
+                         float2* vis_out, int nchan, int ncorr, int nterms, long long npoints) {
   const long long n = (long long)counters[0];
   const int ng = ncorr * nterms;
   for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
     const uint4 w4 = pw[i];
-    if (lra_is_fallback(fb, (int)w4.z)) continue;
+    if (w4.y & 0x80000000u) continue;   // a fallback class: written by the fallback kernel
     const unsigned k = w4.y;
     const int c = (int)(k % (unsigned)nchan);
 #pragma unroll
@@ -92,7 +92,7 @@ int lra_degrid_region_launch(lra_plan* p, const float2* grid, const float* tau, 
   if (rc) return rc;
   lra_degrid_finish_kernel<<<p->sm_count * 8, 256, 0, p->stream>>>(p->pw, p->counters, reinterpret_cast<const float2*>(p->prep),
                                                                   tau, vis_in, vis_out, p->nchan, p->ncorr, p->nterms,
-                                                                  (long long)n, lra_make_fallback_mask(p->tile_x, p->tile, ng));
+                                                                  (long long)n);
   LRA_LAUNCH_CHECK(p);
   return LRA_OK;
 }

@@ -142,11 +142,11 @@ __global__ void __launch_bounds__((NW + 1) * 32) __maxnreg__(LRA_MAXNREG(NW, KS,
       fresh = false;
     }
     const uint32_t lane_base = slots0 + slot * a.slot_bytes + lane_off;
-    const unsigned char* rec = sp + LRA_SLOT_VAL;   // 16 bytes per point: {word, k, S, chunk range}
+    const unsigned char* rec = sp + LRA_SLOT_VAL;   // 16 bytes per point: the pw record {word, k, z, w} (lra_pipe.cuh)
     float* out = reinterpret_cast<float*>(sp + a.out_off);
     // software pipeline over the points of the batch (as in the gridder), four points per reduction
     uint4 pc = *reinterpret_cast<const uint4*>(rec);
-    uint32_t mask = count ? lra_step_mask<NW>(pc.w, warp) : 0u;
+    uint32_t mask = count ? lra_point_mask<NW>(pc.z, pc.w, warp) : 0u;
     lra_load_steps<NW, KS, 0>(T, lane_base + pc.x, mask);
     for (unsigned q0 = 0; q0 < count; q0 += 4) {
       float v[V];
@@ -156,11 +156,11 @@ __global__ void __launch_bounds__((NW + 1) * 32) __maxnreg__(LRA_MAXNREG(NW, KS,
       for (int u = 0; u < 4; ++u) {
         rec += 16;
         pc = *reinterpret_cast<const uint4*>(rec);
-        const uint32_t addr_next = lane_base + pc.x, mask_next = q0 + u + 1 < count ? lra_step_mask<NW>(pc.w, warp) : 0u;
+        const uint32_t addr_next = lane_base + pc.x, mask_next = q0 + u + 1 < count ? lra_point_mask<NW>(pc.z, pc.w, warp) : 0u;
         lra_u64 P1[NG], P2[NG];
 #pragma unroll
         for (int g = 0; g < NG; ++g) P1[g] = P2[g] = 0ull;
-        lra_drun_steps<NW, NG, KS, 0>(P1, P2, G, T, mask, addr_next, mask_next);
+        lra_drun_steps<NW, NG, KS, 0>(P1, P2, G, T, mask, addr_next, lra_opaque(mask_next));
 #pragma unroll
         for (int g = 0; g < NG; ++g) {   // conj(c) * G = (cre*Gre + cim*Gim) + i (cre*Gim - cim*Gre)
           float p1r, p1i, p2r, p2i;

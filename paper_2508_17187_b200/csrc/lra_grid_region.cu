@@ -9,8 +9,8 @@ int lra_grid_launch_ng(lra_plan* p, const lra_region_args& a, const lra_geom& q,
 
 // wt * tau * V of every sorted point in the form the tap loop consumes (reading R6: (wt*tau)*V in fp32).  Grid
 // g = t*ncorr + p belongs to pass g / LRA_NGMAX; the record of sorted position i in a pass of n grids is
-//   n x float4 (vx, vy, -vy, vx), then uint4 (word, c_lo | c_hi << 16, 0, 0)            [lra_point_bytes(n) bytes]
-// with word and the chunk range from lra_work.cu (lra_pipe.cuh).  Every pass but the last holds LRA_NGMAX grids, so
+//   n x float4 (vx, vy, -vy, vx), then uint4 (word, z, w, 0)                            [lra_point_bytes(n) bytes]
+// with word and the step masks / chunk range (z, w) from lra_work.cu (lra_pipe.cuh).  Every pass but the last holds LRA_NGMAX grids, so
 // pass j starts npoints * j * lra_point_bytes(LRA_NGMAX) bytes into `prep`.  One thread per point; the same pass over
 // the weights also gives sumwt[t][p] += wt*tau (fp64 partials per thread, block tree, one atomic per block and grid).
 __global__ void __launch_bounds__(256)
@@ -25,7 +25,7 @@ lra_prepare_kernel(const unsigned long long* __restrict__ counters, const uint4*
   for (int g = 0; g < 16; ++g) acc[g] = 0.0;
   for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
     const uint4 w4 = pw[i];
-    const unsigned k = w4.y;
+    const unsigned k = w4.y & 0x7fffffffu;
     const int c = (int)(k % (unsigned)nchan);
     float2 v[4];
     float w[4];
@@ -52,7 +52,7 @@ lra_prepare_kernel(const unsigned long long* __restrict__ counters, const uint4*
         const int ngp = ng - pass * LRA_NGMAX >= LRA_NGMAX ? LRA_NGMAX : ng - pass * LRA_NGMAX;
         unsigned char* rec = prep + (size_t)npoints * pass * lra_point_bytes(LRA_NGMAX) + (size_t)i * lra_point_bytes(ngp);
         reinterpret_cast<float4*>(rec)[gl] = make_float4(vx, vy, -vy, vx);
-        if (gl == 0) reinterpret_cast<uint4*>(rec)[ngp] = make_uint4(w4.x, w4.w, 0u, 0u);
+        if (gl == 0) reinterpret_cast<uint4*>(rec)[ngp] = make_uint4(w4.x, w4.z, w4.w, 0u);
       }
     }
   }

@@ -37,6 +37,8 @@
 //     never touch the work list and synchronise once per batch, not once per slab.
 // Regions that fit no (NW, KS) take the global-atomic kernel of lra_grid.cu.
 #pragma once
+#include <type_traits>
+
 #include "lra_region.cuh"
 
 // One step of the software pipeline: the FMAs of the CURRENT point on the two pixels this lane owns at the step
@@ -147,8 +149,11 @@ __global__ void __launch_bounds__((NW + 1) * 32) __maxnreg__(LRA_MAXNREG(NW, KS,
     const unsigned char* rec = sp + LRA_SLOT_VAL;
     // software pipeline over the points of the batch: while a step multiplies the taps of point q it reloads its tap
     // registers for point q + 1; the record of point q + 1 is read while point q runs
-    uint2 wc = *reinterpret_cast<const uint2*>(rec + 16 * NG);
-    uint32_t mask = count ? lra_step_mask<NW>(wc.y, warp) : 0u;
+    // (the record's tail is {word, z, w, 0}: 8 bytes are enough up to four consumer warps)
+    using tail_t = typename std::conditional<(NW <= 4), uint2, uint4>::type;
+    auto tail_w = [](const tail_t& t) { if constexpr (NW <= 4) return 0u; else return t.z; };
+    tail_t wc = *reinterpret_cast<const tail_t*>(rec + 16 * NG);
+    uint32_t mask = count ? lra_point_mask<NW>(wc.y, tail_w(wc), warp) : 0u;
     lra_load_steps<NW, KS, 0>(T, lane_base + wc.x, mask);
     for (unsigned q = 0; q < count; ++q) {
       lra_u64 V[NG], W[NG];
@@ -158,9 +163,9 @@ __global__ void __launch_bounds__((NW + 1) * 32) __maxnreg__(LRA_MAXNREG(NW, KS,
         V[g] = v.x; W[g] = v.y;
       }
       rec += PB;
-      wc = *reinterpret_cast<const uint2*>(rec + 16 * NG);
-      const uint32_t addr_next = lane_base + wc.x, mask_next = q + 1 < count ? lra_step_mask<NW>(wc.y, warp) : 0u;
-      lra_run_steps<NW, NG, KS, 0>(acc, V, W, T, mask, addr_next, mask_next);
+      wc = *reinterpret_cast<const tail_t*>(rec + 16 * NG);
+      const uint32_t addr_next = lane_base + wc.x, mask_next = q + 1 < count ? lra_point_mask<NW>(wc.y, tail_w(wc), warp) : 0u;
+      lra_run_steps<NW, NG, KS, 0>(acc, V, W, T, mask, addr_next, lra_opaque(mask_next));
       mask = mask_next;
     }
     lra_mbar_arrive(empty0 + 8 * slot);   // every lane, after its own reads of the slot: no divergent branch in the loop

@@ -61,7 +61,7 @@ struct lra_plan {
   int64_t work_capacity;
   uint32_t* batch;          // batch records (16 words each), grouped by class; an item's are consecutive
   int64_t batch_capacity;   // batches
-  uint4* pw;                // [npoints] per sorted position: {byte offset of its first tap in the batch's slab area, k, S, 0}
+  uint4* pw;                // [npoints] per sorted position: {word, k | fallback << 31, step masks / chunk range} (lra_pipe.cuh)
   int64_t pw_capacity;      // points
   float* prep;              // gridder: wt*tau*V of every sorted point, FFMA2 operand form; degridder: sorted results
   int64_t prep_capacity;    // floats

@@ -133,10 +133,12 @@ __device__ __forceinline__ bool lra_is_fallback(const lra_fallback_mask& m, int 
 //   batch = per_batch consecutive runs of one item: what occupies one slot of a CTA's shared-memory ring.
 //           64 bytes: uint4 {first sorted position, count | flags, runs, tile id}, then the slab offsets of its
 //           runs in 16-byte units (uint32 x 12).  LRA_BATCH_LAST marks the last batch of its item.
-//   pw    = for every sorted position 16 bytes (one TMA granule) {word, k, S, c_lo | c_hi << 16}; word = the byte
+//   pw    = for every sorted position 16 bytes (one TMA granule) {word, k | fallback << 31, z, w}; word = the byte
 //           offset (signed), inside the slot's slab area, of the complex value the lane that owns pixel 0 of the
-//           region would read for this point: 8 * (LRA_GAP + run * stride - off), off = oy*RX + ox; c_lo, c_hi =
-//           first and last chunk of the region that the footprint touches.
+//           region would read for this point: 8 * (LRA_GAP + run * stride - off), off = oy*RX + ox; k = the point's
+//           index in the caller's arrays, bit 31 set if its class takes the fallback kernels; for NW <= 8, byte w of
+//           (z, w) = the step mask of consumer warp w (bit s: chunk NW*s + w lies in [c_lo, c_hi], the first and last
+//           chunk of the region that the footprint touches); for NW = 16, z = c_lo | c_hi << 16.
 // ---------------------------------------------------------------------------------------------------
 #define LRA_BATCH_LAST 0x40000000u
 #define LRA_BATCH_END 0x80000000u

@@ -142,6 +142,23 @@ __device__ __forceinline__ uint32_t lra_step_mask(uint32_t range, int warp) {
   const int s_lo = (c_lo - warp + NW - 1) >> LG, s_hi = (c_hi - warp) >> LG;   // s_hi >= s_lo - 1 >= -1
   return (1u << (s_hi + 1)) - (1u << s_lo);
 }
+// A value behind an opaque move: it lives in an ordinary (not a uniform) register, so that the predicates of the tap
+// loads come from one R2P / per-step LOP3 instead of a uniform extract plus a uniform-to-predicate move each.
+__device__ __forceinline__ uint32_t lra_opaque(uint32_t x) {
+  uint32_t y;
+  asm volatile("mov.b32 %0, %1;" : "=r"(y) : "r"(x));
+  return y;
+}
+
+// Step mask of a point for consumer warp `warp` from the (z, w) words of its pw record (lra_pipe.cuh): a byte picked
+// from the words for NW <= 8 (two uniform instructions), computed from the chunk range for NW = 16.
+template <int NW>
+__device__ __forceinline__ uint32_t lra_point_mask(uint32_t z, uint32_t w, int warp) {
+  if constexpr (NW <= 4) return (z >> (8 * warp)) & 0xffu;
+  else if constexpr (NW == 8) return ((warp < 4 ? z : w) >> (8 * (warp & 3))) & 0xffu;
+  else return lra_step_mask<NW>(z, warp);
+}
+
 // The tap loads of a point, steps [B, KS): predicated on the bits of `mask`.
 template <int NW, int KS, int B>
 __device__ __forceinline__ void lra_load_steps(lra_taps (&T)[KS], uint32_t addr, uint32_t mask) {

@@ -11,7 +11,7 @@ struct lra_work_args {
   int shift_x, shift_y, ntx, tile_x, tile_y, ng;
   uint4* work;
   uint32_t* batch;     // 16 words per batch
-  uint4* pw;           // one 16-byte record per sorted position: {word, k, S, c_lo | c_hi << 16}
+  uint4* pw;           // one 16-byte record per sorted position: {word, k | fallback << 31, masks / chunk range}
   unsigned item_off[LRA_NCLASS], batch_off[LRA_NCLASS];   // FILL pass: first item / batch of every class (from the host)
 };
 
@@ -180,8 +180,18 @@ __global__ void __launch_bounds__(256) lra_work_kernel(const lra_work_args a) {
       const int ix = rc[e].x & 0xffff, iy = rc[e].x >> 16;
       const int ox = ix - ((ix >> a.shift_x) << a.shift_x), oy = iy - ((iy >> a.shift_y) << a.shift_y);
       const int off = oy * q.rx + ox;
-      a.pw[i] = make_uint4((unsigned)(8 * (LRA_GAP + (int)r * q.stride - off)), rc[e].z, rc[e].w & 0xffu,
-                           (unsigned)(off >> 6) | (unsigned)((off + q.span - 1) >> 6) << 16);
+      const int c_lo = off >> 6, c_hi = (off + q.span - 1) >> 6;
+      unsigned mz = (unsigned)c_lo | (unsigned)c_hi << 16, mw = 0u;
+      if (q.nw >= 1 && q.nw <= 8) {   // the step masks of the consumer warps, one byte each (lra_region.cuh)
+        unsigned long long m = 0ull;
+        const int lg = __ffs(q.nw) - 1;   // NW is a power of two
+        for (int w = 0; w < q.nw; ++w) {
+          const int s_lo = (c_lo - w + q.nw - 1) >> lg, s_hi = (c_hi - w) >> lg;   // arithmetic shift: -1 if c_hi < w
+          if (s_hi >= s_lo) m |= (unsigned long long)(((2u << s_hi) - (1u << s_lo)) & 0xffu) << (8 * w);
+        }
+        mz = (unsigned)m; mw = (unsigned)(m >> 32);
+      }
+      a.pw[i] = make_uint4((unsigned)(8 * (LRA_GAP + (int)r * q.stride - off)), rc[e].z | (q.nw == 0 ? 0x80000000u : 0u), mz, mw);
     }
   }
 }
