@@ -16,7 +16,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "liblra_ref.so")
 _SRC = os.path.join(_HERE, "lra_ref.c")
-_SRCS = [_SRC, os.path.join(_HERE, "lra_ref_image.c")]
+_SRCS = [_SRC, os.path.join(_HERE, "lra_ref_image.c"), os.path.join(_HERE, "lra_ref_gain.c")]
 
 SORT_TILE, SORT_TILE_CF = 0, 1
 
@@ -181,3 +181,32 @@ def model_grid(img, corr_x=None, corr_y=None) -> np.ndarray:
     rc = lib().lra_ref_model_grid(C.c_int32(ng), C.c_int32(ny), C.c_int32(nx), _p(img), _p(corr_x), _p(corr_y), _p(out))
     assert rc == 0
     return out
+
+
+def gain_accumulate(vis, model, wt, nbl, bl_index=None, xsum=None, wsum=None):
+    """lra_ref_gain_accumulate (Eq. 19): -> (xsum complex [nbl, ncorr], wsum [nbl, ncorr]), accumulated into if given."""
+    vis = np.ascontiguousarray(vis, dtype=np.complex64)
+    model = np.ascontiguousarray(model, dtype=np.complex64)
+    wt = np.ascontiguousarray(wt, dtype=np.float32)
+    nrow, nchan, ncorr = vis.shape
+    bl_index = None if bl_index is None else np.ascontiguousarray(bl_index, dtype=np.int32)
+    xsum = np.zeros((nbl, ncorr), np.complex128) if xsum is None else xsum
+    wsum = np.zeros((nbl, ncorr), np.float64) if wsum is None else wsum
+    rc = lib().lra_ref_gain_accumulate(C.c_int64(nrow), C.c_int32(nchan), C.c_int32(ncorr), C.c_int32(nbl), _p(bl_index),
+                                       _p(vis), _p(model), _p(wt), _p(xsum), _p(wsum))
+    assert rc == 0
+    return xsum, wsum
+
+
+def gain_solve(nant, ant1, ant2, xsum, wsum, alpha, delta, max_iter, gains0):
+    """lra_ref_gain_solve (Eq. 20, 21): -> (gains complex [nant, ncorr], iterations)."""
+    ant1 = np.ascontiguousarray(ant1, dtype=np.int32)
+    ant2 = np.ascontiguousarray(ant2, dtype=np.int32)
+    xsum = np.ascontiguousarray(xsum, dtype=np.complex128)
+    wsum = np.ascontiguousarray(wsum, dtype=np.float64)
+    g = np.array(gains0, dtype=np.complex128, copy=True, order="C")
+    it = C.c_int32(0)
+    rc = lib().lra_ref_gain_solve(C.c_int32(nant), C.c_int32(len(ant1)), C.c_int32(xsum.shape[1]), _p(ant1), _p(ant2), _p(xsum),
+                                  _p(wsum), C.c_double(alpha), C.c_double(delta), C.c_int32(max_iter), _p(g), C.byref(it))
+    assert rc == 0
+    return g, int(it.value)
