@@ -138,6 +138,30 @@ int lra_image(lra_plan* p, const void* grid_c64, const double* sumwt, const floa
               float* image);
 int lra_model_grid(lra_plan* p, const float* image, const float* corr_x, const float* corr_y, void* grid_c64);
 
+/* The G-Jones solver fed by degridded model visibilities (Sec. 5.1),
+ * readings R21-R23 of DESIGN.md.  Plan-free: device ordinal and cudaStream_t are arguments; both calls only enqueue.
+ *
+ * lra_gain_accumulate, Eq. 19 over one solution interval:
+ *   xsum[b][p] += sum wt * V[k][p] / M[k][p],  wsum[b][p] += sum wt     over the samples k of baseline b with wt > 0, M != 0
+ * (so that X_ij = xsum / wsum, the weighted average, and w_ij = wsum).  Ratio and sums in double.
+ *   bl_index : device int32 [nrow], baseline of every row, or NULL (=> row r belongs to baseline r % nbl)
+ *   vis_c64, model_c64 : device complex64 [nrow][nchan][ncorr] (model = lra_degrid's output without vis_in)
+ *   wt : device float [nrow][nchan][ncorr];  xsum: device complex double [nbl][ncorr];  wsum: device double [nbl][ncorr];
+ *   both ACCUMULATED INTO (caller zeroes them; partitions of the interval may be added call by call).
+ * lra_gain_solve, Eq. 20 / 21 for every correlation independently, from the gains given:
+ *   grad g_i = sum_b [i = ant1: g_j X_b w_b | i = ant2: g_j conj(X_b) w_b] / sum_b |g_j|^2 w_b   (j = the other antenna)
+ *   g_i <- (1 - alpha) g_i + alpha grad g_i    (all antennas from the gains of iteration k)
+ * until max_i |g_i^{k+1} - g_i^k| < delta or max_iter iterations.
+ *   ant1, ant2 : device int32 [nbl];  gains: device complex double [nant][ncorr], in: g^0, out: the solution;
+ *   iters : device int32, the iterations done (largest over the correlations), or NULL.   nant <= 1024.
+ * Errors: LRA_EINVAL, LRA_ECUDA. */
+int lra_gain_accumulate(int32_t device, void* stream, int64_t nrow, int32_t nchan, int32_t ncorr, int32_t nbl,
+                        const int32_t* bl_index, const void* vis_c64, const void* model_c64, const float* wt,
+                        double* xsum, double* wsum);
+int lra_gain_solve(int32_t device, void* stream, int32_t nant, int32_t nbl, int32_t ncorr, const int32_t* ant1,
+                   const int32_t* ant2, const double* xsum, const double* wsum, double alpha, double delta,
+                   int32_t max_iter, double* gains, int32_t* iters);
+
 /* Number of kernel launches the plan has enqueued since creation (for bench.py's gpu_launches). */
 int64_t lra_launch_count(const lra_plan* p);
 

@@ -53,6 +53,8 @@ def lib() -> C.CDLL:
         L.lra_degrid.argtypes = [vp] * 5
         L.lra_image.argtypes = [vp] * 6
         L.lra_model_grid.argtypes = [vp] * 5
+        L.lra_gain_accumulate.argtypes = [i32, vp, i64, i32, i32, i32, vp, vp, vp, vp, vp, vp]
+        L.lra_gain_solve.argtypes = [i32, vp, i32, i32, i32, vp, vp, vp, vp, C.c_double, C.c_double, i32, vp, vp]
         L.lra_launch_count.argtypes = [vp]
         L.lra_launch_count.restype = i64
         L.lra_tap_count.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
@@ -68,7 +70,7 @@ def lib() -> C.CDLL:
 
 
 EXPORTED = ["lra_plan_create", "lra_plan_destroy", "lra_bin", "lra_bin_export", "lra_grid", "lra_degrid", "lra_image",
-            "lra_model_grid",
+            "lra_model_grid", "lra_gain_accumulate", "lra_gain_solve",
             "lra_launch_count", "lra_tap_count", "lra_set_variant", "lra_strerror", "lra_last_cuda_error",
             "lra_diag_fma_tflops", "lra_diag_l2_gbs"]
 
@@ -170,6 +172,28 @@ def lra_model_grid(plan: int, image, corr_x, corr_y, grid):
     import torch
     _check(lib().lra_model_grid(plan, _dev(image, torch.float32, plan), _dev(corr_x, torch.float32, plan),
                                 _dev(corr_y, torch.float32, plan), _dev(grid, torch.complex64, plan)), plan)
+
+
+def lra_gain_accumulate(vis, model, wt, nbl, xsum, wsum, bl_index=None, stream=None):
+    """Eq. 19: xsum complex128 [nbl, ncorr] and wsum float64 [nbl, ncorr] are accumulated into (lra.h)."""
+    import torch
+    nrow, nchan, ncorr = (int(x) for x in vis.shape)
+    if tuple(model.shape) != (nrow, nchan, ncorr) or tuple(wt.shape) != (nrow, nchan, ncorr):
+        raise LraError("vis, model and wt must share the shape [nrow, nchan, ncorr]")
+    if tuple(xsum.shape) != (nbl, ncorr) or tuple(wsum.shape) != (nbl, ncorr):
+        raise LraError("xsum / wsum must be [nbl, ncorr]")
+    _check(lib().lra_gain_accumulate(vis.device.index, stream or 0, nrow, nchan, ncorr, nbl, _dev(bl_index, torch.int32),
+                                     _dev(vis, torch.complex64), _dev(model, torch.complex64), _dev(wt, torch.float32),
+                                     _dev(xsum, torch.complex128), _dev(wsum, torch.float64)))
+
+
+def lra_gain_solve(ant1, ant2, xsum, wsum, alpha, delta, max_iter, gains, iters=None, stream=None):
+    """Eq. 20 / 21: gains complex128 [nant, ncorr] updated in place; iters: int32 CUDA tensor of one element or None."""
+    import torch
+    nant, ncorr = (int(x) for x in gains.shape)
+    _check(lib().lra_gain_solve(gains.device.index, stream or 0, nant, int(ant1.shape[0]), ncorr, _dev(ant1, torch.int32),
+                                _dev(ant2, torch.int32), _dev(xsum, torch.complex128), _dev(wsum, torch.float64), float(alpha),
+                                float(delta), int(max_iter), _dev(gains, torch.complex128), _dev(iters, torch.int32)))
 
 
 def lra_launch_count(plan: int) -> int:

@@ -543,3 +543,58 @@ def test_major_cycle_on_device(B, ref):
     finally:
         run1.close()
         run2.close()
+
+
+# ---------------------------------------------------------------------------------------------------
+# NEXT-4: the G-Jones solver (Eq. 19-21) fed by lra_degrid's model visibilities
+# ---------------------------------------------------------------------------------------------------
+def test_gain_solver_fed_by_degrid(B, ref):
+    """Model visibilities of cfg5-small (degridded model grid), observed = g_i conj(g_j) * model + noise: Eq. 19 sums and the
+    Eq. 20 / 21 iteration against the oracle (double on both sides: 1e-9 relative on the sums over the same complex64
+    inputs, 1e-9 on the gains, identical iteration counts), with and without an explicit baseline index."""
+    wl = W.make_workload(W.small_config(5))
+    c = wl.cfg
+    # the model visibilities: the oracle's prediction in the ABI's precision feeds BOTH solvers; lra_degrid's own
+    # prediction (what a caller would feed) is checked against it first
+    model = ref_for(ref, wl, nterms=1).degrid(wl.uvw, wl.freq, wl.cf_index, wl.model_grid.astype(np.complex128), None).astype(np.complex64)
+    run = run_for(B, wl, nterms=1)
+    try:
+        assert_close(run.degrid(wl.model_grid, None), model, "model visibilities from lra_degrid")
+    finally:
+        run.close()
+    d_model = dev(model)
+    rng = np.random.default_rng(21)
+    nant, nbl = W.N_ANT, W.N_BL
+    a1, a2 = (x.astype(np.int32) for x in np.triu_indices(nant, 1))
+    g = (1 + 0.2 * rng.standard_normal((nant, c.ncorr))) * np.exp(1j * rng.uniform(-1, 1, (nant, c.ncorr)))
+    bl = (np.arange(c.nrow) % nbl).astype(np.int32)
+    vis = (g[a1[bl]][:, None, :] * np.conj(g[a2[bl]])[:, None, :] * model
+           + 0.05 * (rng.standard_normal(model.shape) + 1j * rng.standard_normal(model.shape))).astype(np.complex64)
+    wt = wl.wt.copy()
+    wt[rng.random(wt.shape) < 0.03] = 0.0
+    want_x, want_w = ref.gain_accumulate(vis, model, wt, nbl)
+    for bli in (None, bl[::-1].copy()):
+        xs = torch.zeros((nbl, c.ncorr), dtype=torch.complex128, device="cuda")
+        ws = torch.zeros((nbl, c.ncorr), dtype=torch.float64, device="cuda")
+        if bli is None:
+            B.lra_gain_accumulate(dev(vis), d_model, dev(wt), nbl, xs, ws)
+            wx, ww = want_x, want_w
+        else:
+            B.lra_gain_accumulate(dev(vis), d_model, dev(wt), nbl, xs, ws, bl_index=dev(bli))
+            wx, ww = ref.gain_accumulate(vis, model, wt, nbl, bl_index=bli)
+        torch.cuda.synchronize()
+        assert np.abs(xs.cpu().numpy() - wx).max() <= 1e-9 * np.abs(wx).max()
+        assert np.abs(ws.cpu().numpy() - ww).max() <= 1e-9 * np.abs(ww).max()
+    xs = torch.zeros((nbl, c.ncorr), dtype=torch.complex128, device="cuda")
+    ws = torch.zeros((nbl, c.ncorr), dtype=torch.float64, device="cuda")
+    B.lra_gain_accumulate(dev(vis), d_model, dev(wt), nbl, xs, ws)
+    for alpha, delta, max_iter in ((0.5, 1e-8, 500), (1.0, 0.0, 7), (0.3, 1e-3, 1000)):
+        want_g, want_it = ref.gain_solve(nant, a1, a2, want_x, want_w, alpha, delta, max_iter, np.ones((nant, c.ncorr)))
+        gains = torch.ones((nant, c.ncorr), dtype=torch.complex128, device="cuda")
+        it = torch.zeros(1, dtype=torch.int32, device="cuda")
+        B.lra_gain_solve(dev(a1), dev(a2), xs, ws, alpha, delta, max_iter, gains, it)
+        torch.cuda.synchronize()
+        assert int(it.item()) == want_it
+        assert np.abs(gains.cpu().numpy() - want_g).max() <= 1e-9
+    sol = gains.cpu().numpy()
+    assert np.abs(sol[a1] * np.conj(sol[a2]) - g[a1] * np.conj(g[a2])).max() < 0.05     # the gains are recovered
