@@ -105,16 +105,19 @@ lra_radix_hist_kernel(const uint64_t* __restrict__ keys, long long n, int span, 
   hist[(size_t)threadIdx.x * gridDim.x + blockIdx.x] = h[threadIdx.x];
 }
 
-// Exclusive scan of `m` uint32 in place, one block of 1024 threads.
-__global__ void __launch_bounds__(1024) lra_scan_kernel(uint32_t* __restrict__ a, long long m) {
+// Exclusive scan of the histogram hist[digit][block] in digit-major order, in two small steps instead of one block
+// walking all 256 * blocks entries: block d scans row d in place (exclusive) and leaves the row total in tot[d];
+// lra_scan_tot_kernel then turns tot[] into the exclusive scan over the digits, which the scatter adds.
+__global__ void __launch_bounds__(1024) lra_scan_rows_kernel(uint32_t* __restrict__ hist, int blocks, uint32_t* __restrict__ tot) {
   __shared__ uint32_t warp_tot[32];
   __shared__ uint32_t carry;
+  uint32_t* a = hist + (size_t)blockIdx.x * blocks;
   if (threadIdx.x == 0) carry = 0;
   __syncthreads();
   const int l = threadIdx.x & 31, w = threadIdx.x >> 5;
-  for (long long base = 0; base < m; base += 1024) {
-    long long i = base + threadIdx.x;
-    uint32_t v = i < m ? a[i] : 0u, x = v;
+  for (int base = 0; base < blocks; base += 1024) {
+    const int i = base + threadIdx.x;
+    uint32_t v = i < blocks ? a[i] : 0u, x = v;
     for (int o = 1; o < 32; o <<= 1) {
       uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
       if (l >= o) x += y;
@@ -130,22 +133,38 @@ __global__ void __launch_bounds__(1024) lra_scan_kernel(uint32_t* __restrict__ a
       warp_tot[l] = s - t;  // exclusive
     }
     __syncthreads();
-    uint32_t c = carry;
-    if (i < m) a[i] = c + warp_tot[w] + (x - v);
+    const uint32_t c = carry;
+    if (i < blocks) a[i] = c + warp_tot[w] + (x - v);
     __syncthreads();
     if (threadIdx.x == 1023) carry = c + warp_tot[31] + x;
     __syncthreads();
   }
+  if (threadIdx.x == 0) tot[blockIdx.x] = carry;
+}
+__global__ void __launch_bounds__(LRA_RADIX) lra_scan_tot_kernel(uint32_t* __restrict__ tot) {
+  __shared__ uint32_t warp_tot[8];
+  const int l = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const uint32_t v = tot[threadIdx.x];
+  uint32_t x = v;
+  for (int o = 1; o < 32; o <<= 1) {
+    uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
+    if (l >= o) x += y;
+  }
+  if (l == 31) warp_tot[w] = x;
+  __syncthreads();
+  uint32_t base = 0;
+  for (int ww = 0; ww < w; ++ww) base += warp_tot[ww];
+  tot[threadIdx.x] = base + x - v;
 }
 
 __global__ void __launch_bounds__(256)
 lra_radix_scatter_kernel(const uint64_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in,
                          uint64_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out, long long n, int span,
-                         int shift, const uint32_t* __restrict__ hist_scanned) {
+                         int shift, const uint32_t* __restrict__ hist_scanned, const uint32_t* __restrict__ digit_base) {
   __shared__ uint32_t digit_off[LRA_RADIX];       // running global offset of every digit for this block
   __shared__ uint32_t warp_cnt[8][LRA_RADIX];     // per-warp digit counts of the current round
   const int l = threadIdx.x & 31, w = threadIdx.x >> 5;
-  digit_off[threadIdx.x] = hist_scanned[(size_t)threadIdx.x * gridDim.x + blockIdx.x];
+  digit_off[threadIdx.x] = hist_scanned[(size_t)threadIdx.x * gridDim.x + blockIdx.x] + digit_base[threadIdx.x];
   for (int i = 0; i < 8; ++i) warp_cnt[i][threadIdx.x] = 0;
   __syncthreads();
   long long lo = (long long)blockIdx.x * span, hi = lo + span < n ? lo + span : n;
@@ -274,7 +293,7 @@ int lra_bin_impl(lra_plan* p, int64_t nrow, int32_t nchan, const double* uvw, co
     if (hist_n > p->hist_capacity) {
       LRA_CUDA(p, cudaStreamSynchronize(p->stream));
       p->hist_capacity = 0;
-      if ((rc = lra_regrow(p, &p->hist, hist_n))) return rc;
+      if ((rc = lra_regrow(p, &p->hist, hist_n + LRA_RADIX))) return rc;   // + the per-digit totals
       p->hist_capacity = hist_n;
     }
     int cur = 0;
@@ -282,10 +301,12 @@ int lra_bin_impl(lra_plan* p, int64_t nrow, int32_t nchan, const double* uvw, co
       int shift = 8 * ps;
       lra_radix_hist_kernel<<<sblocks, 256, 0, p->stream>>>(p->skey[cur], n, (int)span, shift, p->hist);
       LRA_LAUNCH_CHECK(p);
-      lra_scan_kernel<<<1, 1024, 0, p->stream>>>(p->hist, hist_n);
+      lra_scan_rows_kernel<<<LRA_RADIX, 1024, 0, p->stream>>>(p->hist, sblocks, p->hist + hist_n);
+      LRA_LAUNCH_CHECK(p);
+      lra_scan_tot_kernel<<<1, LRA_RADIX, 0, p->stream>>>(p->hist + hist_n);
       LRA_LAUNCH_CHECK(p);
       lra_radix_scatter_kernel<<<sblocks, 256, 0, p->stream>>>(p->skey[cur], p->sval[cur], p->skey[cur ^ 1],
-                                                               p->sval[cur ^ 1], n, (int)span, shift, p->hist);
+                                                               p->sval[cur ^ 1], n, (int)span, shift, p->hist, p->hist + hist_n);
       LRA_LAUNCH_CHECK(p);
       cur ^= 1;
     }
