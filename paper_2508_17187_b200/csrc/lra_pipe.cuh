@@ -90,7 +90,10 @@ __host__ __device__ inline lra_geom lra_make_geom(int S, int tile_x, int tile_y,
 #endif
   for (int pass = 0; pass < 2 && q.nw == 0; ++pass) {
     const int lim = pass == 0 && LRA_KS_PREF < lra_ks_max(ngp) ? LRA_KS_PREF : lra_ks_max(ngp);
-    for (int nw = 1; nw <= 16; nw <<= 1) {
+#ifndef LRA_NW_MIN
+#define LRA_NW_MIN 2   // consumer warps per CTA at least: with one, half of the resident warps are producers (measured on cfg3: 1 -> 2: -0.6 ms gridder, -0.4 ms degridder; 4: worse)
+#endif
+    for (int nw = LRA_NW_MIN; nw <= 16; nw <<= 1) {
       int ks = (chunks + nw - 1) / nw;
       if (ks == 5 || ks == 7) ++ks;   // the kernels are instantiated for KS = 1, 2, 3, 4, 6, 8
       if (ks > lim) continue;
