@@ -16,7 +16,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "liblra_ref.so")
 _SRC = os.path.join(_HERE, "lra_ref.c")
-_SRCS = [_SRC, os.path.join(_HERE, "lra_ref_image.c"), os.path.join(_HERE, "lra_ref_gain.c")]
+_SRCS = [_SRC, os.path.join(_HERE, "lra_ref_image.c"), os.path.join(_HERE, "lra_ref_gain.c"),
+         os.path.join(_HERE, "lra_ref_cf.c")]
 
 SORT_TILE, SORT_TILE_CF = 0, 1
 
@@ -210,3 +211,18 @@ def gain_solve(nant, ant1, ant2, xsum, wsum, alpha, delta, max_iter, gains0):
                                   _p(wsum), C.c_double(alpha), C.c_double(delta), C.c_int32(max_iter), _p(g), C.byref(it))
     assert rc == 0
     return g, int(it.value)
+
+
+def cf(n_img, oversampling, fov_rad, support, taper=None, w_lambda=0.0, aterm=None, normalise=True) -> np.ndarray:
+    """lra_ref_cf (Table 1): one CF of `support` pixels as complex128 [(S os), (S os)] (oracle/lra_ref_cf.c)."""
+    taper = None if taper is None else np.ascontiguousarray(taper, dtype=np.float64)
+    aterm = None if aterm is None else np.ascontiguousarray(aterm, dtype=np.complex128)
+    assert taper is None or taper.shape == (n_img,)
+    assert aterm is None or aterm.shape == (n_img, n_img)
+    so = support * oversampling
+    out = np.empty((so, so), dtype=np.complex128)
+    rc = lib().lra_ref_cf(C.c_int32(n_img), C.c_int32(oversampling), C.c_double(fov_rad), _p(taper), C.c_double(w_lambda),
+                          _p(aterm), C.c_int32(support), C.c_int32(1 if normalise else 0), _p(out))
+    if rc != 0:
+        raise RuntimeError(f"lra_ref_cf rc={rc}")
+    return out
