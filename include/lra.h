@@ -57,7 +57,8 @@ typedef struct {
   int32_t n_cf;           /* number of kernels in the CF table                                                 */
   const int32_t* cf_support; /* host [n_cf]: support S_c in pixels, odd, 1 <= S_c <= 129                        */
   const int64_t* cf_offset;  /* host [n_cf]: element (complex64) offset of kernel c inside cf_data              */
-  const void* cf_data;    /* host, complex64: kernel c is (S_c*os)^2 samples, row-major, v slow; sample m of a
+  const void* cf_data;    /* host OR device (e.g. lra_cf_generate's output; the unified address space tells which),
+                             complex64: kernel c is (S_c*os)^2 samples, row-major, v slow; sample m of a
                              row sits (m - c0)/os pixels from the kernel centre, c0 = h*os + (os-1-os/2) [R3]   */
   int32_t device;         /* CUDA device ordinal                                                               */
   void* stream;           /* cudaStream_t all work of this plan is enqueued on (NULL = legacy default stream)  */
@@ -161,6 +162,46 @@ int lra_gain_accumulate(int32_t device, void* stream, int64_t nrow, int32_t ncha
 int lra_gain_solve(int32_t device, void* stream, int32_t nant, int32_t nbl, int32_t ncorr, const int32_t* ant1,
                    const int32_t* ant2, const double* xsum, const double* wsum, double alpha, double delta,
                    int32_t max_iter, double* gains, int32_t* iters);
+
+/* ---- PreCompute: construction of the CF table on the device ----------------------
+ * Table 1 configures a CF as the uv-plane convolution of the terms that are ON -- the anti-aliasing
+ * prolate-spheroidal taper PS, the A-term, the W-term -- "constructed from ideal kernels", computed once in
+ * PreCompute or on demand by the CFCache.  The convolution is evaluated as the Fourier
+ * transform of the product of the terms in the image plane (readings R24-R26 in DESIGN.md):
+ *   img[m][l] = taper[l] taper[m] * aterm[a_c][m][l] * e^{2 pi i w_c (sqrt(1 - l^2 - m^2) - 1)},
+ *               l = (l_index - n_img/2) fov_rad / n_img, likewise m; sqrt of a negative number taken as 0;
+ *   K_c[j][i] = sum_m sum_l img[m][l] e^{-2 pi i (off_j (m - n_img/2) + off_i (l - n_img/2)) / n_img},
+ *               off_j = (j - c0)/os, c0 as in lra_plan_desc.cf_data (= the n_img*os-point DFT of the zero-padded image,
+ *               cropped to the (S_c os)^2 samples about the centre);
+ *   normalise != 0: K_c is scaled (complex) so that its samples sum to os^2.
+ * A term is OFF when its pointer is NULL: taper NULL = PSTerm OFF, aterm NULL (n_aterm 0) = ATerm OFF, cf_w NULL = WTerm
+ * OFF; the six rows of Table 1 are the six combinations with at least one term ON.  Arithmetic is fp64, the result is
+ * rounded once to complex64.  A caller grows a table "with usage" by calling again with the new kernels
+ * and offsets past the old ones. */
+typedef struct {
+  int32_t n_img;             /* image raster is n_img x n_img over the field of view, 2 <= n_img <= 512                */
+  int32_t oversampling;      /* os, as in lra_plan_desc                                                               */
+  double fov_rad;            /* field of view spanned by the raster, in direction-cosine units (radians), > 0         */
+  const double* taper;       /* DEVICE double [n_img] or NULL: separable image-plane taper                            */
+  int32_t n_aterm;           /* number of A-term patterns (0 = ATerm OFF)                                             */
+  const void* aterm;         /* DEVICE complex64 [n_aterm][n_img][n_img] (m slow, l fast) or NULL                     */
+  int32_t n_cf;              /* kernels to build                                                                      */
+  const int32_t* cf_support; /* host [n_cf]: support S_c, odd, 1 <= S_c <= 129                                        */
+  const int64_t* cf_offset;  /* host [n_cf]: element offset of kernel c in cf_data (regions must not overlap)         */
+  const double* cf_w;        /* host [n_cf]: w of kernel c in wavelengths, or NULL (WTerm OFF)                        */
+  const int32_t* cf_aterm;   /* host [n_cf]: A-term pattern of kernel c, or NULL (pattern 0 for all)                  */
+  int32_t normalise;         /* != 0: scale every kernel to sum os^2 [R12]                                            */
+  int32_t device;            /* CUDA device ordinal                                                                   */
+  void* stream;              /* cudaStream_t the work is enqueued on                                                  */
+} lra_cf_desc;
+
+/* Writes the n_cf kernels into cf_data (DEVICE complex64, caller-owned, large enough for every offset + (S_c os)^2).
+ * Allocates and frees its own work buffers (<= ~256 MB) and synchronises the stream before returning.
+ * Errors: LRA_EINVAL (bad argument; also a kernel whose samples sum to 0 or NaN when normalise != 0 -- the other kernels
+ * are still written), LRA_ENOMEM, LRA_ECUDA (lra_cf_last_cuda_error() returns the cudaError_t of this thread's last
+ * failure). */
+int lra_cf_generate(const lra_cf_desc* desc, void* cf_data_c64);
+int lra_cf_last_cuda_error(void);
 
 /* Number of kernel launches the plan has enqueued since creation (for bench.py's gpu_launches). */
 int64_t lra_launch_count(const lra_plan* p);

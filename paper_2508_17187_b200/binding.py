@@ -31,6 +31,13 @@ class lra_plan_desc(C.Structure):
                 ("device", C.c_int32), ("stream", C.c_void_p), ("tile_x", C.c_int32)]
 
 
+class lra_cf_desc(C.Structure):
+    _fields_ = [("n_img", C.c_int32), ("oversampling", C.c_int32), ("fov_rad", C.c_double), ("taper", C.c_void_p),
+                ("n_aterm", C.c_int32), ("aterm", C.c_void_p), ("n_cf", C.c_int32), ("cf_support", C.c_void_p),
+                ("cf_offset", C.c_void_p), ("cf_w", C.c_void_p), ("cf_aterm", C.c_void_p), ("normalise", C.c_int32),
+                ("device", C.c_int32), ("stream", C.c_void_p)]
+
+
 _lib = None
 
 
@@ -55,6 +62,8 @@ def lib() -> C.CDLL:
         L.lra_model_grid.argtypes = [vp] * 5
         L.lra_gain_accumulate.argtypes = [i32, vp, i64, i32, i32, i32, vp, vp, vp, vp, vp, vp]
         L.lra_gain_solve.argtypes = [i32, vp, i32, i32, i32, vp, vp, vp, vp, C.c_double, C.c_double, i32, vp, vp]
+        L.lra_cf_generate.argtypes = [C.POINTER(lra_cf_desc), vp]
+        L.lra_cf_last_cuda_error.restype = C.c_int
         L.lra_launch_count.argtypes = [vp]
         L.lra_launch_count.restype = i64
         L.lra_tap_count.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
@@ -70,7 +79,7 @@ def lib() -> C.CDLL:
 
 
 EXPORTED = ["lra_plan_create", "lra_plan_destroy", "lra_bin", "lra_bin_export", "lra_grid", "lra_degrid", "lra_image",
-            "lra_model_grid", "lra_gain_accumulate", "lra_gain_solve",
+            "lra_model_grid", "lra_gain_accumulate", "lra_gain_solve", "lra_cf_generate", "lra_cf_last_cuda_error",
             "lra_launch_count", "lra_tap_count", "lra_set_variant", "lra_strerror", "lra_last_cuda_error",
             "lra_diag_fma_tflops", "lra_diag_l2_gbs"]
 
@@ -107,14 +116,22 @@ def _host(a: np.ndarray, dtype) -> np.ndarray:
 
 def lra_plan_create(nx, ny, ncorr, nterms, oversampling, scale_u, scale_v, cf_support, cf_offset, cf_data,
                     tile=0, sort_mode=LRA_SORT_TILE_CF, device=0, stream=None, tile_x=0) -> int:
-    """-> opaque plan handle (int).  cf_* are HOST numpy arrays (lra.h: lra_plan_desc).  tile = 0: the library's
+    """-> opaque plan handle (int).  cf_support / cf_offset are HOST numpy arrays; cf_data is a HOST numpy array or a
+    CUDA complex64 tensor (e.g. lra_cf_generate's output) (lra.h: lra_plan_desc).  tile = 0: the library's
     default 8 x 8 tiles; tile_x = 0 with tile != 0: square tiles.  stream: a CUDA stream handle (int), 0 / None = the
     default stream."""
     sup = _host(cf_support, np.int32)
     off = _host(cf_offset, np.int64)
-    dat = _host(cf_data, np.complex64)
+    if isinstance(cf_data, np.ndarray):
+        dat = _host(cf_data, np.complex64)
+        dat_ptr = dat.ctypes.data
+    else:
+        import torch
+        if cf_data.device.index != int(device):
+            raise LraError(f"cf_data on cuda:{cf_data.device.index}, plan on cuda:{int(device)}")
+        dat_ptr = _dev(cf_data, torch.complex64)
     d = lra_plan_desc(nx, ny, ncorr, nterms, oversampling, tile, sort_mode, float(scale_u), float(scale_v), len(sup),
-                      sup.ctypes.data, off.ctypes.data, dat.ctypes.data, device, stream or 0, tile_x)
+                      sup.ctypes.data, off.ctypes.data, dat_ptr, device, stream or 0, tile_x)
     h = C.c_void_p()
     _check(lib().lra_plan_create(C.byref(h), C.byref(d)))
     _plan_device[h.value] = int(device)
@@ -194,6 +211,42 @@ def lra_gain_solve(ant1, ant2, xsum, wsum, alpha, delta, max_iter, gains, iters=
     _check(lib().lra_gain_solve(gains.device.index, stream or 0, nant, int(ant1.shape[0]), ncorr, _dev(ant1, torch.int32),
                                 _dev(ant2, torch.int32), _dev(xsum, torch.complex128), _dev(wsum, torch.float64), float(alpha),
                                 float(delta), int(max_iter), _dev(gains, torch.complex128), _dev(iters, torch.int32)))
+
+
+def lra_cf_generate(cf_data, n_img, oversampling, fov_rad, cf_support, cf_offset, taper=None, aterm=None, cf_w=None,
+                    cf_aterm=None, normalise=True, stream=None):
+    """Table 1 / PreCompute (lra.h: lra_cf_generate).  cf_data: CUDA complex64 flat tensor written at cf_offset;
+    taper: CUDA float64 [n_img] or None; aterm: CUDA complex64 [n_aterm, n_img, n_img] or None; cf_support, cf_offset,
+    cf_w (or None), cf_aterm (or None): HOST arrays [n_cf]."""
+    import torch
+    sup = _host(cf_support, np.int32)
+    off = _host(cf_offset, np.int64)
+    w = None if cf_w is None else _host(cf_w, np.float64)
+    ia = None if cf_aterm is None else _host(cf_aterm, np.int32)
+    n_cf = len(sup)
+    if len(off) != n_cf or (w is not None and len(w) != n_cf) or (ia is not None and len(ia) != n_cf):
+        raise LraError("cf_support, cf_offset, cf_w and cf_aterm must have one entry per kernel")
+    if n_cf and int((off + (sup.astype(np.int64) * oversampling) ** 2).max()) > cf_data.numel():
+        raise LraError("cf_data is too small for the offsets given")
+    dev = cf_data.device.index
+    for t in (taper, aterm):
+        if t is not None and t.device.index != dev:
+            raise LraError("taper / aterm must be on cf_data's device")
+    if taper is not None and tuple(taper.shape) != (n_img,):
+        raise LraError(f"taper must be [n_img], got {tuple(taper.shape)}")
+    if aterm is not None and (aterm.dim() != 3 or tuple(aterm.shape[1:]) != (n_img, n_img)):
+        raise LraError(f"aterm must be [n_aterm, n_img, n_img], got {tuple(aterm.shape)}")
+    d = lra_cf_desc(n_img, oversampling, float(fov_rad), _dev(taper, torch.float64), 0 if aterm is None else int(aterm.shape[0]),
+                    _dev(aterm, torch.complex64), n_cf, sup.ctypes.data, off.ctypes.data, None if w is None else w.ctypes.data,
+                    None if ia is None else ia.ctypes.data, 1 if normalise else 0, dev, stream or 0)
+    rc = lib().lra_cf_generate(C.byref(d), _dev(cf_data, torch.complex64))
+    if rc != LRA_OK:
+        raise LraError(f"{lib().lra_strerror(rc).decode()} (cudaError {lib().lra_cf_last_cuda_error()})")
+
+
+def lra_cf_last_cuda_error() -> int:
+    """cudaError_t of the calling thread's last lra_cf_generate failure (0 = none)."""
+    return int(lib().lra_cf_last_cuda_error())
 
 
 def lra_launch_count(plan: int) -> int:

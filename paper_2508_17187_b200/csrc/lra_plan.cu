@@ -109,7 +109,7 @@ extern "C" int lra_plan_create(lra_plan** out, const lra_plan_desc* d) {
     int S = p->cf_support[c];
     int64_t n_in = (int64_t)S * p->os * S * p->os;
     const float2* src = (const float2*)d->cf_data + d->cf_offset[c];
-    CK(cudaMemcpyAsync(staging, src, (size_t)n_in * sizeof(float2), cudaMemcpyHostToDevice, p->stream));
+    CK(cudaMemcpyAsync(staging, src, (size_t)n_in * sizeof(float2), cudaMemcpyDefault, p->stream));   // host or device table
     int64_t n_out = (int64_t)p->os * p->os * (p->slab_stride[c] / 2);
     int blocks = (int)((n_out + 255) / 256);
     if (blocks > 4096) blocks = 4096;
