@@ -378,6 +378,130 @@ int lra_ref_degrid_points(const lra_ref_desc* d, int64_t nrow, int32_t nchan, co
   return 0;
 }
 
+/* ---------------------------------------------------------------------------------------------- */
+/* The general kernel of Eq. 27 and the sparse Mueller matrix of CFs:
+ *     c_ij = CF_ij(nu, w, t)  f(ds_i - ds_j)  e^{2 pi i [s_o - (s(P) + ds_i + ds_j)] . u}
+ * Readings R27-R29: the exponent lost its ". u" in print (G1); u is the uv coordinate of the GRID PIXEL the
+ * tap lands on, u_X = (X - nx/2) / scale_u wavelengths (v likewise), so the factor is a phase gradient across the kernel;
+ * the caller supplies, per row, an index into a table of (f, dl, dm) with (dl, dm) = s_o - (s(P) + ds_i + ds_j) in
+ * direction cosines (Table 2's four modes are four ways of filling that table).  A Mueller element e = (grid plane p_e,
+ * visibility correlation q_e) has its own kernel index per visibility point: gridding adds CF_e (x) [wt v]_{q_e} to plane
+ * p_e, degridding adds conj(c_e) . G_{p_e} to correlation q_e.  sumwt counts wt * tau on the DIAGONAL elements only (a
+ * leakage term adds no weight); validity (R4) is per element, since the support is.
+ *   elem_grid, elem_corr [n_elem]; cf_index[e] -> int32 [nrow][nchan] (NULL: kernel 0); vis, wt [nrow][nchan][ncorr_vis];
+ *   po_table [n_po][3] double (NULL: f = 1, no gradient), po_index [nrow] (NULL: entry 0); grid [nterms][d->ncorr][ny][nx]. */
+static void po_factor(const lra_ref_desc* d, const double* po_table, const int32_t* po_index, int64_t r, int32_t X,
+                      int32_t Y, double sign, double* fr, double* fi) {
+  if (!po_table) { *fr = 1.0; *fi = 0.0; return; }
+  const double* e = po_table + 3 * (po_index ? po_index[r] : 0);
+  double ux = (double)(X - d->nx / 2) / d->scale_u, vy = (double)(Y - d->ny / 2) / d->scale_v;
+  double ph = sign * 6.283185307179586476925286766559 * (e[1] * ux + e[2] * vy);
+  *fr = e[0] * cos(ph);
+  *fi = e[0] * sin(ph);
+}
+
+int lra_ref_grid_awp(const lra_ref_desc* d, int64_t nrow, int32_t nchan, const double* uvw, const double* freq,
+                     int32_t n_elem, const int32_t* elem_grid, const int32_t* elem_corr, const int32_t* const* cf_index,
+                     int32_t ncorr_vis, const float* vis, const float* wt, const float* tau, const double* po_table,
+                     const int32_t* po_index, double* grid, double* sumwt) {
+  const int32_t ng = d->ncorr, nt = d->nterms, nx = d->nx, ny = d->ny;
+  for (int64_t r = 0; r < nrow; ++r)
+    for (int32_t c = 0; c < nchan; ++c) {
+      int64_t k = r * nchan + c;
+      for (int32_t e = 0; e < n_elem; ++e) {
+        int32_t p = elem_grid[e], qc = elem_corr[e];
+        if (p < 0 || p >= ng || qc < 0 || qc >= ncorr_vis) return 1;
+        ref_point q = locate(d, uvw, freq, cf_index ? cf_index[e] : 0, nchan, r, c);
+        if (!q.valid) continue;
+        int32_t S = d->cf_support[q.cf], h = (S - 1) / 2;
+        for (int32_t t = 0; t < nt; ++t) {
+          double tw = tau ? (double)tau[c * nt + t] : 1.0;
+          double w = (double)wt[k * ncorr_vis + qc] * tw;
+          double vr = w * (double)vis[2 * (k * ncorr_vis + qc)], vi = w * (double)vis[2 * (k * ncorr_vis + qc) + 1];
+          if (sumwt && p == qc) sumwt[t * ng + p] += w;
+          double* g = grid + 2 * ((int64_t)(t * ng + p) * ny * nx);
+          for (int32_t j = -h; j <= h; ++j)
+            for (int32_t i = -h; i <= h; ++i) {
+              const float* cfp = tap_ptr(d, &q, j, i);
+              double fr, fi;
+              po_factor(d, po_table, po_index, r, q.ix + i, q.iy + j, 1.0, &fr, &fi);
+              double cr = (double)cfp[0] * fr - (double)cfp[1] * fi, ci = (double)cfp[0] * fi + (double)cfp[1] * fr;
+              double* px = g + 2 * ((int64_t)(q.iy + j) * nx + (q.ix + i));
+              px[0] += cr * vr - ci * vi;
+              px[1] += cr * vi + ci * vr;
+            }
+        }
+      }
+    }
+  return 0;
+}
+
+/* vis_out[nrow][nchan][ncorr_vis] complex double = (vis_in or 0) - sum_e [q_e = q] sum_t tau sum_taps conj(c_e) G[t][p_e] */
+int lra_ref_degrid_awp(const lra_ref_desc* d, int64_t nrow, int32_t nchan, const double* uvw, const double* freq,
+                       int32_t n_elem, const int32_t* elem_grid, const int32_t* elem_corr, const int32_t* const* cf_index,
+                       int32_t ncorr_vis, const double* grid, const float* tau, const double* po_table,
+                       const int32_t* po_index, const float* vis_in, double* vis_out) {
+  const int32_t ng = d->ncorr, nt = d->nterms, nx = d->nx, ny = d->ny;
+  for (int64_t r = 0; r < nrow; ++r)
+    for (int32_t c = 0; c < nchan; ++c) {
+      int64_t k = r * nchan + c;
+      for (int32_t qc = 0; qc < ncorr_vis; ++qc) vis_out[2 * (k * ncorr_vis + qc)] = vis_out[2 * (k * ncorr_vis + qc) + 1] = 0.0;
+      for (int32_t e = 0; e < n_elem; ++e) {
+        int32_t p = elem_grid[e], qc = elem_corr[e];
+        if (p < 0 || p >= ng || qc < 0 || qc >= ncorr_vis) return 1;
+        ref_point q = locate(d, uvw, freq, cf_index ? cf_index[e] : 0, nchan, r, c);
+        if (!q.valid) continue;
+        int32_t S = d->cf_support[q.cf], h = (S - 1) / 2;
+        for (int32_t t = 0; t < nt; ++t) {
+          double tw = tau ? (double)tau[c * nt + t] : 1.0;
+          const double* g = grid + 2 * ((int64_t)(t * ng + p) * ny * nx);
+          double sr = 0.0, si = 0.0;
+          for (int32_t j = -h; j <= h; ++j)
+            for (int32_t i = -h; i <= h; ++i) {
+              const float* cfp = tap_ptr(d, &q, j, i);
+              double fr, fi;
+              po_factor(d, po_table, po_index, r, q.ix + i, q.iy + j, 1.0, &fr, &fi);
+              /* conj(c f e^{i ph}) */
+              double cr = (double)cfp[0] * fr - (double)cfp[1] * fi, ci = -((double)cfp[0] * fi + (double)cfp[1] * fr);
+              const double* px = g + 2 * ((int64_t)(q.iy + j) * nx + (q.ix + i));
+              sr += cr * px[0] - ci * px[1];
+              si += cr * px[1] + ci * px[0];
+            }
+          vis_out[2 * (k * ncorr_vis + qc)] += tw * sr;
+          vis_out[2 * (k * ncorr_vis + qc) + 1] += tw * si;
+        }
+      }
+      for (int32_t qc = 0; qc < ncorr_vis; ++qc) {
+        double ar = vis_out[2 * (k * ncorr_vis + qc)], ai = vis_out[2 * (k * ncorr_vis + qc) + 1];
+        if (vis_in) {
+          ar = (double)vis_in[2 * (k * ncorr_vis + qc)] - ar;
+          ai = (double)vis_in[2 * (k * ncorr_vis + qc) + 1] - ai;
+        }
+        vis_out[2 * (k * ncorr_vis + qc)] = ar;
+        vis_out[2 * (k * ncorr_vis + qc) + 1] = ai;
+      }
+    }
+  return 0;
+}
+
+/* dst (+)= f e^{sign 2 pi i (dl u_X + dm v_Y)} src, all planes: the same factor applied to a whole grid (a group of
+ * visibilities that share one pointing term; Table 2 "mosaic imaging, no PO correction"). */
+int lra_ref_phase_gradient(const lra_ref_desc* d, int32_t nplanes, const double* src, double f, double dl, double dm,
+                           int32_t conjugate, int32_t accumulate, double* dst) {
+  double e[3] = {f, dl, dm};
+  for (int32_t g = 0; g < nplanes; ++g)
+    for (int32_t Y = 0; Y < d->ny; ++Y)
+      for (int32_t X = 0; X < d->nx; ++X) {
+        double fr, fi;
+        po_factor(d, e, 0, 0, X, Y, conjugate ? -1.0 : 1.0, &fr, &fi);
+        int64_t o = 2 * (((int64_t)g * d->ny + Y) * d->nx + X);
+        double a = src[o], b = src[o + 1];
+        double rr = a * fr - b * fi, ri = a * fi + b * fr;
+        if (accumulate) { dst[o] += rr; dst[o + 1] += ri; } else { dst[o] = rr; dst[o + 1] = ri; }
+      }
+  return 0;
+}
+
 int lra_ref_max_threads(void) {
 #ifdef _OPENMP
   return omp_get_max_threads();

@@ -120,6 +120,56 @@ class RefPlan:
         assert rc == 0
         return out
 
+    def _awp(self, elems, cf_indices, po_table, po_index):
+        eg = np.ascontiguousarray([e[0] for e in elems], dtype=np.int32)
+        ec = np.ascontiguousarray([e[1] for e in elems], dtype=np.int32)
+        keep = [None if a is None else np.ascontiguousarray(a, dtype=np.int32) for a in (cf_indices or [None] * len(elems))]
+        ptrs = (C.c_void_p * len(elems))(*[None if a is None else a.ctypes.data for a in keep])
+        po_table = None if po_table is None else np.ascontiguousarray(po_table, dtype=np.float64).reshape(-1, 3)
+        po_index = None if po_index is None else np.ascontiguousarray(po_index, dtype=np.int32)
+        return eg, ec, keep, ptrs, po_table, po_index
+
+    def grid_awp(self, uvw, freq, elems, cf_indices, vis, wt, tau=None, po_table=None, po_index=None):
+        """lra_ref_grid_awp (Eq. 27 + Mueller elements).  elems: [(grid plane, visibility correlation)]; cf_indices: one
+        int32 [nrow, nchan] (or None) per element; vis, wt: [nrow, nchan, ncorr_vis]; -> (grid, sumwt)."""
+        uvw, freq, _, nrow, nchan = self._geom(uvw, freq, None)
+        eg, ec, keep, ptrs, po_table, po_index = self._awp(elems, cf_indices, po_table, po_index)
+        vis = np.ascontiguousarray(vis, dtype=np.complex64)
+        wt = np.ascontiguousarray(wt, dtype=np.float32)
+        tau = None if tau is None else np.ascontiguousarray(tau, dtype=np.float32)
+        grid = np.zeros((self.nterms, self.ncorr, self.ny, self.nx), dtype=np.complex128)
+        sumwt = np.zeros((self.nterms, self.ncorr), dtype=np.float64)
+        rc = lib().lra_ref_grid_awp(C.byref(self.d), C.c_int64(nrow), C.c_int32(nchan), _p(uvw), _p(freq), C.c_int32(len(eg)),
+                                    _p(eg), _p(ec), ptrs, C.c_int32(vis.shape[2]), _p(vis), _p(wt), _p(tau), _p(po_table),
+                                    _p(po_index), _p(grid), _p(sumwt))
+        assert rc == 0
+        return grid, sumwt
+
+    def degrid_awp(self, uvw, freq, elems, cf_indices, ncorr_vis, grid, tau=None, po_table=None, po_index=None, vis_in=None):
+        """lra_ref_degrid_awp -> complex128 [nrow, nchan, ncorr_vis]."""
+        uvw, freq, _, nrow, nchan = self._geom(uvw, freq, None)
+        eg, ec, keep, ptrs, po_table, po_index = self._awp(elems, cf_indices, po_table, po_index)
+        grid = np.ascontiguousarray(grid, dtype=np.complex128)
+        tau = None if tau is None else np.ascontiguousarray(tau, dtype=np.float32)
+        vis_in = None if vis_in is None else np.ascontiguousarray(vis_in, dtype=np.complex64)
+        out = np.empty((nrow, nchan, ncorr_vis), dtype=np.complex128)
+        rc = lib().lra_ref_degrid_awp(C.byref(self.d), C.c_int64(nrow), C.c_int32(nchan), _p(uvw), _p(freq), C.c_int32(len(eg)),
+                                      _p(eg), _p(ec), ptrs, C.c_int32(ncorr_vis), _p(grid), _p(tau), _p(po_table),
+                                      _p(po_index), _p(vis_in), _p(out))
+        assert rc == 0
+        return out
+
+    def phase_gradient(self, src, f, dl, dm, conjugate=False, dst=None):
+        """lra_ref_phase_gradient: dst (+)= f e^{+-2 pi i (dl u + dm v)} src over all planes of src [..., ny, nx]."""
+        src = np.ascontiguousarray(src, dtype=np.complex128)
+        nplanes = int(np.prod(src.shape[:-2], dtype=np.int64)) if src.ndim > 2 else 1
+        acc = dst is not None
+        out = np.ascontiguousarray(dst, dtype=np.complex128).copy() if acc else np.empty_like(src)
+        rc = lib().lra_ref_phase_gradient(C.byref(self.d), C.c_int32(nplanes), _p(src), C.c_double(f), C.c_double(dl),
+                                          C.c_double(dm), C.c_int32(1 if conjugate else 0), C.c_int32(1 if acc else 0), _p(out))
+        assert rc == 0
+        return out
+
     def grid_pixels(self, uvw, freq, cf_index, vis, wt, tau, pix, nthreads=0):
         uvw, freq, cf_index, nrow, nchan = self._geom(uvw, freq, cf_index)
         vis = np.ascontiguousarray(vis, dtype=np.complex64)
