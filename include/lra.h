@@ -203,6 +203,48 @@ typedef struct {
 int lra_cf_generate(const lra_cf_desc* desc, void* cf_data_c64);
 int lra_cf_last_cuda_error(void);
 
+/* ---- the data-dependent terms of Eq. 27 and per-element Mueller CFs ----------------
+ *   c_ij(P, nu, w) = CF_ij(nu, w, t)  f(ds_i - ds_j)  e^{2 pi i [s_o - (s(P) + ds_i + ds_j)] . u}      (Eq. 27)
+ * "the rest of the terms ... represents the data-dependent perturbations applied on-the-fly"; s_o, s(P) and
+ * the antenna pointing offsets ds_i are input meta-data (Table 2).  Readings R27-R29: u is the
+ * uv coordinate of the grid pixel a tap lands on, u_X = (X - nx/2)/scale_u, v_Y = (Y - ny/2)/scale_v (wavelengths); the
+ * caller reduces the meta-data to a table po_table[n_po][3] = (f, dl, dm), (dl, dm) = s_o - (s(P) + ds_i + ds_j) in
+ * direction cosines, and a per-row index po_index[nrow] into it.  Gridding uses c f e^{+2 pi i (dl u_X + dm v_Y)},
+ * degridding its conjugate; sumwt carries no f [R6].  Table 2's modes: single pointing without PO = the plain calls;
+ * mosaic without PO = one call per pointing with po_index NULL (every row uses entry 0: the tiled kernels run unchanged
+ * and the factor is applied to the grid once); with PO correction = per-row entries (direct kernels).
+ *   po_table : HOST double [n_po][3], 1 <= n_po <= 2^20, finite;  po_index : DEVICE int32 [nrow] or NULL; rows whose index
+ *   is outside [0, n_po) are skipped (they add nothing to the grid; their model visibility is 0).  Other arguments as
+ *   lra_grid / lra_degrid.  The first call with po_index NULL allocates one scratch grid in the plan.
+ * lra_phase_gradient: dst (+)= f e^{+-2 pi i (dl u_X + dm v_Y)} src on all nterms*ncorr planes of a grid (- with
+ *   conjugate != 0; += with accumulate != 0; src == dst allowed without accumulate).
+ * Errors: LRA_EINVAL, LRA_ESTATE (before lra_bin), LRA_ENOMEM, LRA_ECUDA. */
+int lra_phase_gradient(lra_plan* p, const void* src_c64, double f, double dl, double dm, int32_t conjugate,
+                       int32_t accumulate, void* dst_c64);
+int lra_grid_po(lra_plan* p, const void* vis_c64, const float* wt, const float* tau, int32_t n_po, const double* po_table,
+                const int32_t* po_index, void* grid_c64, double* sumwt);
+int lra_degrid_po(lra_plan* p, const void* grid_c64, const float* tau, int32_t n_po, const double* po_table,
+                  const int32_t* po_index, const void* vis_in_c64, void* vis_out_c64);
+
+/* Sparse Mueller matrix of CFs: element e = (grid plane elem_grid[e], visibility correlation elem_corr[e])
+ * has its own kernel index per visibility point, cf_index[e] (HOST array of n_elem DEVICE pointers to int32 [nrow][nchan],
+ * NULL entry = kernel 0).  Gridding adds CF_e (x) [wt V]_{elem_corr[e]} to plane elem_grid[e]; degridding subtracts (adds,
+ * without vis_in) conj(c_e) . G_{elem_grid[e]} from correlation elem_corr[e].  Only the elements listed are computed (the
+ * matrix "can be configured to include only terms that are significant").  sumwt [ngrid] receives wt * tau of the DIAGONAL
+ * elements (elem_grid == elem_corr) only [R29].  The plan must have ncorr = nterms = 1 (one plane of geometry); every
+ * element re-bins it (lra_bin with the element's indices), so the plan is left binned for the last element.
+ *   vis, wt : DEVICE [nrow][nchan][ncorr_vis]; grid : DEVICE complex64 [ngrid][ny][nx]; tau : DEVICE [nchan] or NULL;
+ *   n_po = 0 disables the pointing term (po_table, po_index as above otherwise); n_elem <= 16, ncorr_vis, ngrid <= 4.
+ * Both synchronise the stream before returning (they free their gather buffers). */
+int lra_grid_mueller(lra_plan* p, int64_t nrow, int32_t nchan, const double* uvw_m, const double* freq_hz, int32_t n_elem,
+                     const int32_t* elem_grid, const int32_t* elem_corr, const int32_t* const* cf_index, int32_t ncorr_vis,
+                     const void* vis_c64, const float* wt, const float* tau, int32_t n_po, const double* po_table,
+                     const int32_t* po_index, int32_t ngrid, void* grid_c64, double* sumwt);
+int lra_degrid_mueller(lra_plan* p, int64_t nrow, int32_t nchan, const double* uvw_m, const double* freq_hz, int32_t n_elem,
+                       const int32_t* elem_grid, const int32_t* elem_corr, const int32_t* const* cf_index, int32_t ncorr_vis,
+                       int32_t ngrid, const void* grid_c64, const float* tau, int32_t n_po, const double* po_table,
+                       const int32_t* po_index, const void* vis_in_c64, void* vis_out_c64);
+
 /* Number of kernel launches the plan has enqueued since creation (for bench.py's gpu_launches). */
 int64_t lra_launch_count(const lra_plan* p);
 

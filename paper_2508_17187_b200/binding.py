@@ -63,6 +63,11 @@ def lib() -> C.CDLL:
         L.lra_gain_accumulate.argtypes = [i32, vp, i64, i32, i32, i32, vp, vp, vp, vp, vp, vp]
         L.lra_gain_solve.argtypes = [i32, vp, i32, i32, i32, vp, vp, vp, vp, C.c_double, C.c_double, i32, vp, vp]
         L.lra_cf_generate.argtypes = [C.POINTER(lra_cf_desc), vp]
+        L.lra_phase_gradient.argtypes = [vp, vp, C.c_double, C.c_double, C.c_double, i32, i32, vp]
+        L.lra_grid_po.argtypes = [vp, vp, vp, vp, i32, vp, vp, vp, vp]
+        L.lra_degrid_po.argtypes = [vp, vp, vp, i32, vp, vp, vp, vp]
+        L.lra_grid_mueller.argtypes = [vp, i64, i32, vp, vp, i32, vp, vp, vp, i32, vp, vp, vp, i32, vp, vp, i32, vp, vp]
+        L.lra_degrid_mueller.argtypes = [vp, i64, i32, vp, vp, i32, vp, vp, vp, i32, i32, vp, vp, i32, vp, vp, vp, vp]
         L.lra_cf_last_cuda_error.restype = C.c_int
         L.lra_launch_count.argtypes = [vp]
         L.lra_launch_count.restype = i64
@@ -80,6 +85,7 @@ def lib() -> C.CDLL:
 
 EXPORTED = ["lra_plan_create", "lra_plan_destroy", "lra_bin", "lra_bin_export", "lra_grid", "lra_degrid", "lra_image",
             "lra_model_grid", "lra_gain_accumulate", "lra_gain_solve", "lra_cf_generate", "lra_cf_last_cuda_error",
+            "lra_phase_gradient", "lra_grid_po", "lra_degrid_po", "lra_grid_mueller", "lra_degrid_mueller",
             "lra_launch_count", "lra_tap_count", "lra_set_variant", "lra_strerror", "lra_last_cuda_error",
             "lra_diag_fma_tflops", "lra_diag_l2_gbs"]
 
@@ -242,6 +248,80 @@ def lra_cf_generate(cf_data, n_img, oversampling, fov_rad, cf_support, cf_offset
     rc = lib().lra_cf_generate(C.byref(d), _dev(cf_data, torch.complex64))
     if rc != LRA_OK:
         raise LraError(f"{lib().lra_strerror(rc).decode()} (cudaError {lib().lra_cf_last_cuda_error()})")
+
+
+def _po(po_table, po_index, plan, nrow=None):
+    import torch
+    t = _host(po_table, np.float64).reshape(-1, 3)
+    if po_index is not None and nrow is not None and tuple(po_index.shape) != (nrow,):
+        raise LraError(f"po_index must be [nrow], got {tuple(po_index.shape)}")
+    return t, len(t), _dev(po_index, torch.int32, plan)
+
+
+def lra_phase_gradient(plan: int, src, f, dl, dm, dst, conjugate=False, accumulate=False):
+    """dst (+)= f e^{+-2 pi i (dl u_X + dm v_Y)} src over all planes (lra.h: lra_phase_gradient)."""
+    import torch
+    if src.shape != dst.shape:
+        raise LraError("src and dst must have the same shape")
+    _check(lib().lra_phase_gradient(plan, _dev(src, torch.complex64, plan), float(f), float(dl), float(dm),
+                                    1 if conjugate else 0, 1 if accumulate else 0, _dev(dst, torch.complex64, plan)), plan)
+
+
+def lra_grid_po(plan: int, vis, wt, tau, po_table, po_index, grid, sumwt=None):
+    """lra_grid with the pointing term of Eq. 27: po_table HOST [n_po, 3] = (f, dl, dm); po_index CUDA int32 [nrow] or None."""
+    import torch
+    t, n_po, pi = _po(po_table, po_index, plan, int(vis.shape[0]))
+    _check(lib().lra_grid_po(plan, _dev(vis, torch.complex64, plan), _dev(wt, torch.float32, plan), _dev(tau, torch.float32, plan),
+                             n_po, t.ctypes.data, pi, _dev(grid, torch.complex64, plan), _dev(sumwt, torch.float64, plan)), plan)
+
+
+def lra_degrid_po(plan: int, grid, tau, po_table, po_index, vis_in, vis_out):
+    import torch
+    t, n_po, pi = _po(po_table, po_index, plan, int(vis_out.shape[0]))
+    _check(lib().lra_degrid_po(plan, _dev(grid, torch.complex64, plan), _dev(tau, torch.float32, plan), n_po, t.ctypes.data, pi,
+                               _dev(vis_in, torch.complex64, plan), _dev(vis_out, torch.complex64, plan)), plan)
+
+
+def _mueller(plan, elems, cf_indices):
+    import torch
+    eg = _host([e[0] for e in elems], np.int32)
+    ec = _host([e[1] for e in elems], np.int32)
+    if len(cf_indices) != len(elems):
+        raise LraError("one cf_index (or None) per element")
+    ptrs = (C.c_void_p * len(elems))(*[_dev(a, torch.int32, plan) for a in cf_indices])
+    return eg, ec, ptrs
+
+
+def lra_grid_mueller(plan: int, uvw_m, freq_hz, elems, cf_indices, vis, wt, tau, grid, sumwt=None, po_table=None, po_index=None):
+    """Sparse Mueller gridding (lra.h: lra_grid_mueller).  elems: [(grid plane, visibility correlation)]; cf_indices: one
+    CUDA int32 [nrow, nchan] (or None) per element; vis, wt CUDA [nrow, nchan, ncorr_vis]; grid CUDA complex64 [ngrid, ny, nx]."""
+    import torch
+    f = _host(freq_hz, np.float64)
+    nrow, nchan = int(uvw_m.shape[0]), len(f)
+    if tuple(vis.shape[:2]) != (nrow, nchan) or vis.shape != wt.shape or grid.dim() != 3:
+        raise LraError("vis / wt must be [nrow, nchan, ncorr_vis], grid [ngrid, ny, nx]")
+    eg, ec, ptrs = _mueller(plan, elems, cf_indices)
+    t, n_po, pi = (None, 0, None) if po_table is None else _po(po_table, po_index, plan, nrow)
+    _check(lib().lra_grid_mueller(plan, nrow, nchan, _dev(uvw_m, torch.float64, plan), f.ctypes.data, len(eg), eg.ctypes.data,
+                                  ec.ctypes.data, ptrs, int(vis.shape[2]), _dev(vis, torch.complex64, plan),
+                                  _dev(wt, torch.float32, plan), _dev(tau, torch.float32, plan), n_po,
+                                  None if t is None else t.ctypes.data, pi, int(grid.shape[0]), _dev(grid, torch.complex64, plan),
+                                  _dev(sumwt, torch.float64, plan)), plan)
+
+
+def lra_degrid_mueller(plan: int, uvw_m, freq_hz, elems, cf_indices, grid, tau, vis_in, vis_out, po_table=None, po_index=None):
+    import torch
+    f = _host(freq_hz, np.float64)
+    nrow, nchan = int(uvw_m.shape[0]), len(f)
+    if tuple(vis_out.shape[:2]) != (nrow, nchan) or grid.dim() != 3 or (vis_in is not None and vis_in.shape != vis_out.shape):
+        raise LraError("vis must be [nrow, nchan, ncorr_vis], grid [ngrid, ny, nx]")
+    eg, ec, ptrs = _mueller(plan, elems, cf_indices)
+    t, n_po, pi = (None, 0, None) if po_table is None else _po(po_table, po_index, plan, nrow)
+    _check(lib().lra_degrid_mueller(plan, nrow, nchan, _dev(uvw_m, torch.float64, plan), f.ctypes.data, len(eg), eg.ctypes.data,
+                                    ec.ctypes.data, ptrs, int(vis_out.shape[2]), int(grid.shape[0]),
+                                    _dev(grid, torch.complex64, plan), _dev(tau, torch.float32, plan), n_po,
+                                    None if t is None else t.ctypes.data, pi, _dev(vis_in, torch.complex64, plan),
+                                    _dev(vis_out, torch.complex64, plan)), plan)
 
 
 def lra_cf_last_cuda_error() -> int:

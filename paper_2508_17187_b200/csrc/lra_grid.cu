@@ -103,6 +103,12 @@ lra_grid_atomic_kernel(const lra_rec* __restrict__ rec, const unsigned long long
   }
 }
 
+int lra_sumwt_launch(lra_plan* p, const float* wt, const float* tau, double* sumwt) {
+  lra_sumwt_kernel<<<p->sm_count * 4, 256, 0, p->stream>>>(p->rec, p->counters, wt, tau, p->nchan, p->ncorr, p->nterms, sumwt);
+  LRA_LAUNCH_CHECK(p);
+  return LRA_OK;
+}
+
 // defined in lra_grid_region.cu
 int lra_grid_region_launch(lra_plan* p, const float2* vis, const float* wt, const float* tau, float2* grid, double* sumwt);
 

@@ -73,6 +73,10 @@ struct lra_plan {
   float2* fft_work;         // complex scratch [nterms*ncorr][ny][nx]
   int fft_plan;             // cufftHandle (0 = none yet)
   bool fft_ready;
+  // ---- Eq. 27 terms (lra_awp.cu) ----
+  void* awp_buf;            // gradient phasor table (nx + ny complex) and the uploaded (f, dl, dm) table
+  size_t awp_bytes;
+  float2* po_scratch;       // one grid [nterms*ncorr][ny][nx], allocated by the first call that needs it
   // ---- misc ----
   int32_t grid_variant, degrid_variant;
   int64_t launches;

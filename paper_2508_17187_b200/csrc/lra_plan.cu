@@ -134,7 +134,7 @@ extern "C" int lra_plan_destroy(lra_plan* p) {
   cudaStreamSynchronize(p->stream);
   lra_fft_release(p);
   void* ptrs[] = {p->slabs, p->d_cf_support, p->d_slab_off, p->ix, p->iy, p->fx, p->fy, p->key, p->skey[0], p->skey[1],
-                  p->sval[0], p->sval[1], p->hist, p->tile_start, p->rec, p->urec, p->counters, p->d_su, p->d_sv, p->work, p->batch, p->pw, p->prep};
+                  p->sval[0], p->sval[1], p->hist, p->tile_start, p->rec, p->urec, p->counters, p->d_su, p->d_sv, p->work, p->batch, p->pw, p->prep, p->awp_buf, p->po_scratch};
   for (void* q : ptrs)
     if (q) cudaFree(q);
   for (int s = 0; s < LRA_NAUX; ++s) {
