@@ -157,38 +157,92 @@ __global__ void __launch_bounds__(LRA_RADIX) lra_scan_tot_kernel(uint32_t* __res
   tot[threadIdx.x] = base + x - v;
 }
 
+// One pass of the least-significant-digit radix sort: block b moves the keys of its span [b*span, (b+1)*span) to their
+// places, 4,096 keys at a time.  The keys of a round are ranked (stably: by warp, sub-round, lane), staged in shared memory
+// in digit order, and only then written out: every digit's keys of a round form one run of consecutive addresses (16 keys
+// = 128 bytes on average) instead of 4,096 isolated 8-byte writes.
+#define LRA_SORT_TILE_KEYS 4096
+#define LRA_SORT_ITEMS 16   // keys per thread and round: warp w owns keys [w*512, (w+1)*512) of the round
+struct lra_scatter_smem {
+  uint64_t keys[LRA_SORT_TILE_KEYS];
+  uint32_t vals[LRA_SORT_TILE_KEYS];
+  uint32_t warp_cnt[8][LRA_RADIX];   // running count of (warp, digit); after the prefix step: keys of lower warps
+  uint32_t digit_off[LRA_RADIX];     // running global offset of every digit for this block
+  uint32_t lstart[LRA_RADIX];        // first staged position of the digit in this round
+  uint32_t gdelta[LRA_RADIX];        // global position minus staged position
+  uint32_t wsum[8];
+};
+
 __global__ void __launch_bounds__(256)
 lra_radix_scatter_kernel(const uint64_t* __restrict__ keys_in, const uint32_t* __restrict__ vals_in,
                          uint64_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out, long long n, int span,
                          int shift, const uint32_t* __restrict__ hist_scanned, const uint32_t* __restrict__ digit_base) {
-  __shared__ uint32_t digit_off[LRA_RADIX];       // running global offset of every digit for this block
-  __shared__ uint32_t warp_cnt[8][LRA_RADIX];     // per-warp digit counts of the current round
-  const int l = threadIdx.x & 31, w = threadIdx.x >> 5;
-  digit_off[threadIdx.x] = hist_scanned[(size_t)threadIdx.x * gridDim.x + blockIdx.x] + digit_base[threadIdx.x];
-  for (int i = 0; i < 8; ++i) warp_cnt[i][threadIdx.x] = 0;
+  extern __shared__ __align__(16) unsigned char lra_scatter_raw[];
+  lra_scatter_smem& sm = *reinterpret_cast<lra_scatter_smem*>(lra_scatter_raw);
+  const int t = threadIdx.x, l = t & 31, w = t >> 5;
+  sm.digit_off[t] = hist_scanned[(size_t)t * gridDim.x + blockIdx.x] + digit_base[t];
+  for (int i = 0; i < 8; ++i) sm.warp_cnt[i][t] = 0;
   __syncthreads();
-  long long lo = (long long)blockIdx.x * span, hi = lo + span < n ? lo + span : n;
-  for (long long base = lo; base < hi; base += 256) {
-    long long i = base + threadIdx.x;
-    bool act = i < hi;
-    uint64_t key = act ? keys_in[i] : 0;
-    uint32_t val = act ? vals_in[i] : 0;
-    unsigned d = (unsigned)(key >> shift) & 255u;
-    // lanes of this warp with the same digit (inactive lanes get a digit of their own: 256 + lane)
-    unsigned peers = __match_any_sync(0xffffffffu, act ? d : 256u + l);
-    unsigned rank = __popc(peers & ((1u << l) - 1u));
-    if (act && rank == 0) warp_cnt[w][d] = __popc(peers);
-    __syncthreads();
-    if (act) {
-      uint32_t pos = digit_off[d] + rank;
-      for (int ww = 0; ww < w; ++ww) pos += warp_cnt[ww][d];
-      keys_out[pos] = key;
-      vals_out[pos] = val;
+  const long long lo = (long long)blockIdx.x * span, hi = lo + span < n ? lo + span : n;
+  for (long long base = lo; base < hi; base += LRA_SORT_TILE_KEYS) {
+    const int cnt = (int)(hi - base < LRA_SORT_TILE_KEYS ? hi - base : LRA_SORT_TILE_KEYS);
+    uint64_t key[LRA_SORT_ITEMS];
+    uint32_t val[LRA_SORT_ITEMS];
+    uint32_t rank[LRA_SORT_ITEMS];   // rank among the warp's keys of the same digit, digit in the top byte
+#pragma unroll
+    for (int r = 0; r < LRA_SORT_ITEMS; ++r) {
+      const int i = w * (32 * LRA_SORT_ITEMS) + r * 32 + l;
+      const bool act = i < cnt;
+      key[r] = act ? keys_in[base + i] : 0;
+      val[r] = act ? vals_in[base + i] : 0;
+    }
+#pragma unroll
+    for (int r = 0; r < LRA_SORT_ITEMS; ++r) {
+      const int i = w * (32 * LRA_SORT_ITEMS) + r * 32 + l;
+      const bool act = i < cnt;
+      const unsigned d = (unsigned)(key[r] >> shift) & 255u;
+      // lanes of this warp with the same digit (inactive lanes get a digit of their own: 256 + lane)
+      const unsigned peers = __match_any_sync(0xffffffffu, act ? d : 256u + l);
+      const unsigned below = __popc(peers & ((1u << l) - 1u));
+      uint32_t old = 0;
+      if (act && below == 0) { old = sm.warp_cnt[w][d]; sm.warp_cnt[w][d] = old + __popc(peers); }
+      old = __shfl_sync(0xffffffffu, old, __ffs(peers) - 1);
+      rank[r] = (old + below) | (d << 24) | (act ? 0u : 0x800000u);
+      __syncwarp();
     }
     __syncthreads();
-    uint32_t tot = 0;
-    for (int ww = 0; ww < 8; ++ww) { tot += warp_cnt[ww][threadIdx.x]; warp_cnt[ww][threadIdx.x] = 0; }
-    digit_off[threadIdx.x] += tot;
+    {   // thread t = digit t: keys of lower warps, then the exclusive scan of the digit totals over the block
+      uint32_t run = 0;
+#pragma unroll
+      for (int ww = 0; ww < 8; ++ww) { const uint32_t c = sm.warp_cnt[ww][t]; sm.warp_cnt[ww][t] = run; run += c; }
+      uint32_t x = run;
+      for (int o = 1; o < 32; o <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, x, o); if (l >= o) x += y; }
+      if (l == 31) sm.wsum[w] = x;
+      __syncthreads();
+      uint32_t before = 0;
+      for (int ww = 0; ww < w; ++ww) before += sm.wsum[ww];
+      const uint32_t start = before + x - run;
+      sm.lstart[t] = start;
+      sm.gdelta[t] = sm.digit_off[t] - start;
+      sm.digit_off[t] += run;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < LRA_SORT_ITEMS; ++r) {
+      if (rank[r] & 0x800000u) continue;
+      const unsigned d = rank[r] >> 24;
+      const uint32_t pos = sm.lstart[d] + sm.warp_cnt[w][d] + (rank[r] & 0x7fffffu);
+      sm.keys[pos] = key[r];
+      sm.vals[pos] = val[r];
+    }
+    __syncthreads();
+    for (int i = t; i < cnt; i += 256) {
+      const uint64_t k = sm.keys[i];
+      const uint32_t pos = sm.gdelta[(unsigned)(k >> shift) & 255u] + (uint32_t)i;
+      keys_out[pos] = k;
+      vals_out[pos] = sm.vals[i];
+    }
+    for (int i = 0; i < 8; ++i) sm.warp_cnt[i][t] = 0;
     __syncthreads();
   }
 }
@@ -296,6 +350,7 @@ int lra_bin_impl(lra_plan* p, int64_t nrow, int32_t nchan, const double* uvw, co
       if ((rc = lra_regrow(p, &p->hist, hist_n + LRA_RADIX))) return rc;   // + the per-digit totals
       p->hist_capacity = hist_n;
     }
+    LRA_CUDA(p, cudaFuncSetAttribute(lra_radix_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(lra_scatter_smem)));
     int cur = 0;
     for (int ps = 0; ps < passes; ++ps) {
       int shift = 8 * ps;
@@ -305,7 +360,7 @@ int lra_bin_impl(lra_plan* p, int64_t nrow, int32_t nchan, const double* uvw, co
       LRA_LAUNCH_CHECK(p);
       lra_scan_tot_kernel<<<1, LRA_RADIX, 0, p->stream>>>(p->hist + hist_n);
       LRA_LAUNCH_CHECK(p);
-      lra_radix_scatter_kernel<<<sblocks, 256, 0, p->stream>>>(p->skey[cur], p->sval[cur], p->skey[cur ^ 1],
+      lra_radix_scatter_kernel<<<sblocks, 256, sizeof(lra_scatter_smem), p->stream>>>(p->skey[cur], p->sval[cur], p->skey[cur ^ 1],
                                                                p->sval[cur ^ 1], n, (int)span, shift, p->hist, p->hist + hist_n);
       LRA_LAUNCH_CHECK(p);
       cur ^= 1;
