@@ -13,7 +13,7 @@ int lra_degrid_launch_ng(lra_plan* p, const lra_region_args& a, const lra_geom& 
 // per point.
 __global__ void __launch_bounds__(256)
 lra_degrid_finish_kernel(const uint4* __restrict__ pw, const unsigned long long* __restrict__ counters,
-                         const float2* __restrict__ res, const float* __restrict__ tau, const float2* vis_in,
+                         const float2* __restrict__ res, const float* __restrict__ tau, bool residual,
                          float2* vis_out, int nchan, int ncorr, int nterms, long long npoints) {
   const long long n = (long long)counters[0];
   const int ng = ncorr * nterms;
@@ -35,8 +35,9 @@ lra_degrid_finish_kernel(const uint4* __restrict__ pw, const unsigned long long*
         vy = fmaf(tw, v.y, vy);
       }
       float2 o = make_float2(vx, vy);
-      if (vis_in) {
-        const float2 vi = vis_in[(size_t)k * ncorr + p];
+      if (residual) {   // lra_degrid_init_kernel has copied vis_in to vis_out: reading it back here touches the sector that
+                        // is written next, where a read of vis_in[k] would fetch a second one
+        const float2 vi = vis_out[(size_t)k * ncorr + p];
         o = make_float2(vi.x - vx, vi.y - vy);
       }
       vis_out[(size_t)k * ncorr + p] = o;
@@ -91,7 +92,7 @@ int lra_degrid_region_launch(lra_plan* p, const float2* grid, const float* tau, 
   }
   if (rc) return rc;
   lra_degrid_finish_kernel<<<p->sm_count * 8, 256, 0, p->stream>>>(p->pw, p->counters, reinterpret_cast<const float2*>(p->prep),
-                                                                  tau, vis_in, vis_out, p->nchan, p->ncorr, p->nterms,
+                                                                  tau, vis_in != nullptr, vis_out, p->nchan, p->ncorr, p->nterms,
                                                                   (long long)n);
   LRA_LAUNCH_CHECK(p);
   return LRA_OK;
