@@ -271,6 +271,13 @@ lra_record_kernel(const uint32_t* __restrict__ perm, const unsigned long long* _
   rec[i] = urec[perm[i]];
 }
 
+__global__ void __launch_bounds__(256)
+lra_scale_from_host_kernel(const double* __restrict__ h, double* __restrict__ su, double* __restrict__ sv, int nchan) {
+  const int i = blockIdx.x * 256 + threadIdx.x;
+  if (i < nchan) su[i] = h[i];
+  else if (i < 2 * nchan) sv[i - nchan] = h[i];
+}
+
 template <typename T>
 static int lra_regrow(lra_plan* p, T** ptr, size_t count) {
   if (*ptr) { cudaFree(*ptr); *ptr = nullptr; }
@@ -306,16 +313,28 @@ int lra_bin_impl(lra_plan* p, int64_t nrow, int32_t nchan, const double* uvw, co
     if ((rc = lra_regrow(p, &p->d_sv, nchan))) return rc;
     p->su_capacity = nchan;
   }
+  if (nchan > p->h_scale_capacity) {
+    LRA_CUDA(p, cudaStreamSynchronize(p->stream));
+    if (p->h_scale) { cudaFreeHost(p->h_scale); p->h_scale = nullptr; p->h_scale_capacity = 0; }
+    LRA_CUDA(p, cudaHostAlloc(&p->h_scale, (size_t)2 * nchan * sizeof(double), cudaHostAllocMapped));
+    p->h_scale_capacity = nchan;
+  }
   // per-channel scale, formed on the host in IEEE double: su[c] = (freq[c] / c) * scale_u  [R2]
-  std::vector<double> su(nchan), sv(nchan);
+  // (lra_bin ends with a host synchronisation, so the previous call's kernel has read h_scale long ago; the table goes to
+  // the device through a kernel reading pinned, mapped memory rather than a cudaMemcpy: see lra_work.cu)
+  double* su = p->h_scale;
+  double* sv = p->h_scale + nchan;
   for (int c = 0; c < nchan; ++c) {
     volatile double lam_inv = freq_host[c] / 299792458.0;
     volatile double a = lam_inv * p->scale_u, b = lam_inv * p->scale_v;
     su[c] = a; sv[c] = b;
   }
-  LRA_CUDA(p, cudaMemcpyAsync(p->d_su, su.data(), nchan * sizeof(double), cudaMemcpyHostToDevice, p->stream));
-  LRA_CUDA(p, cudaMemcpyAsync(p->d_sv, sv.data(), nchan * sizeof(double), cudaMemcpyHostToDevice, p->stream));
-  // (pageable source: the runtime stages the bytes before cudaMemcpyAsync returns, so su / sv may go out of scope)
+  if (nrow * (int64_t)nchan > 0) {   // (an empty call enqueues nothing that reads h_scale, and ends without a synchronisation)
+    double* hd = nullptr;
+    LRA_CUDA(p, cudaHostGetDevicePointer(&hd, p->h_scale, 0));
+    lra_scale_from_host_kernel<<<(2 * nchan + 255) / 256, 256, 0, p->stream>>>(hd, p->d_su, p->d_sv, nchan);
+    LRA_LAUNCH_CHECK(p);
+  }
   LRA_CUDA(p, cudaMemsetAsync(p->counters, 0, LRA_TICKET0 * sizeof(unsigned long long), p->stream));
 
   unsigned long long per_tile = 1;

@@ -77,6 +77,11 @@ struct lra_plan {
   void* awp_buf;            // gradient phasor table (nx + ny complex) and the uploaded (f, dl, dm) table
   size_t awp_bytes;
   float2* po_scratch;       // one grid [nterms*ncorr][ny][nx], allocated by the first call that needs it
+  // ---- pinned, mapped host memory for the few words that cross the bus inside lra_bin: written / read by tiny kernels,
+  //      so that they never queue behind a caller's bulk transfers on the copy engines ----
+  unsigned long long* h_counts;   // [256] list sizes, device -> host
+  double* h_scale;                // [2 * h_scale_capacity] per-channel scales, host -> device
+  int32_t h_scale_capacity;
   // ---- misc ----
   int32_t grid_variant, degrid_variant;
   int64_t launches;

@@ -100,6 +100,7 @@ extern "C" int lra_plan_create(lra_plan** out, const lra_plan_desc* d) {
   }
   CK(cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming));
   CK(cudaMalloc(&p->tile_start, (size_t)(p->ntiles + 1) * sizeof(uint32_t)));
+  CK(cudaHostAlloc(&p->h_counts, 256 * sizeof(unsigned long long), cudaHostAllocMapped));
   CK(cudaMemcpyAsync(p->d_cf_support, p->cf_support.data(), (size_t)d->n_cf * sizeof(int32_t), cudaMemcpyHostToDevice, p->stream));
   CK(cudaMemcpyAsync(p->d_slab_off, p->slab_off.data(), (size_t)d->n_cf * sizeof(int64_t), cudaMemcpyHostToDevice, p->stream));
   // Kernels are staged one at a time through a buffer sized for the largest, so the device never holds two
@@ -142,6 +143,8 @@ extern "C" int lra_plan_destroy(lra_plan* p) {
     if (p->ev_join[s]) cudaEventDestroy(p->ev_join[s]);
   }
   if (p->ev_fork) cudaEventDestroy(p->ev_fork);
+  if (p->h_counts) cudaFreeHost(p->h_counts);
+  if (p->h_scale) cudaFreeHost(p->h_scale);
   delete p;
   return LRA_OK;
 }

@@ -196,6 +196,11 @@ __global__ void __launch_bounds__(256) lra_work_kernel(const lra_work_args a) {
   }
 }
 
+__global__ void __launch_bounds__(256) lra_counts_to_host_kernel(const unsigned long long* __restrict__ src, unsigned long long* dst) {
+  dst[threadIdx.x] = src[threadIdx.x];
+  __threadfence_system();
+}
+
 template <typename T>
 static int lra_grow(lra_plan* p, T** ptr, int64_t* cap, int64_t need) {
   if (need <= *cap) return LRA_OK;
@@ -223,9 +228,15 @@ int lra_build_work(lra_plan* p) {
   lra_work_kernel<false><<<blocks, 256, 0, p->stream>>>(a);
   LRA_LAUNCH_CHECK(p);
   static_assert(LRA_CNT_BATCHES == LRA_CNT_ITEMS + 128 && LRA_CNT_BATCH_OFF == LRA_CNT_ITEM_OFF + 128, "counter layout");
-  unsigned long long h[256];
-  LRA_CUDA(p, cudaMemcpyAsync(h, p->counters + LRA_CNT_ITEMS, sizeof h, cudaMemcpyDeviceToHost, p->stream));
+  // the list sizes go to the host through a kernel that writes pinned, mapped memory: a cudaMemcpy would queue on the
+  // copy engine behind whatever bulk transfer the caller has in flight on another stream (measured: 29 ms per step in
+  // bench.py's pipelined end-to-end loop)
+  unsigned long long* hd = nullptr;
+  LRA_CUDA(p, cudaHostGetDevicePointer(&hd, p->h_counts, 0));
+  lra_counts_to_host_kernel<<<1, 256, 0, p->stream>>>(p->counters + LRA_CNT_ITEMS, hd);
+  LRA_LAUNCH_CHECK(p);
   LRA_CUDA(p, cudaStreamSynchronize(p->stream));   // the one host synchronisation of lra_bin: the list sizes
+  const unsigned long long* h = p->h_counts;
   int64_t items = 0, batches = 0;
   for (int c = 0; c < LRA_NCLASS; ++c) {
     p->n_items[c] = (int64_t)h[c];
