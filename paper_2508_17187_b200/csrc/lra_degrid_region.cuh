@@ -93,14 +93,17 @@ __device__ __forceinline__ void lra_drun_steps(lra_u64 (&P1)[NG], lra_u64 (&P2)[
 }
 
 template <int NW, int KS, int NG>
-__global__ void __launch_bounds__((NW + 1) * 32) __maxnreg__(LRA_MAXNREG(NW, KS, NG, true)) lra_degrid_region_kernel(const lra_region_args a) {
+__global__ void __launch_bounds__((lra_cw(NW) + 1) * 32) __maxnreg__(LRA_MAXNREG(NW, KS, NG, true)) lra_degrid_region_kernel(const lra_region_args a) {
   extern __shared__ __align__(128) unsigned char smem[];
   const int lane = threadIdx.x & 31;
   const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);   // provably warp-uniform: uniform registers
   const uint32_t sbase = lra_smem_u32(smem);
   const uint32_t full0 = sbase, empty0 = sbase + 128, slots0 = sbase + LRA_RING_HDR;
   lra_region_ring_init<NW>(a, smem, full0, empty0);
-  if (warp == NW) {
+  constexpr int PS = NW == 1 ? LRA_PS_WARPS : 1;   // point-split warps (lra_cw in lra_pipe.cuh)
+  const int pwarp = PS > 1 ? 0 : warp;             // which chunks of the region this warp owns
+  const unsigned first = PS > 1 ? (unsigned)warp : 0u;   // its first point of a batch
+  if (warp == lra_cw(NW)) {
     lra_region_producer<NW, NG>(a, a.prep, 16, smem + LRA_RING_HDR, full0, empty0, slots0);
     return;
   }
@@ -112,7 +115,7 @@ __global__ void __launch_bounds__((NW + 1) * 32) __maxnreg__(LRA_MAXNREG(NW, KS,
   for (int s = 0; s < KS; ++s) T[s].v[0] = T[s].v[1] = T[s].v[2] = T[s].v[3] = 0u;
   bool fresh = true;
   uint32_t slot = 0, par = 0;
-  const uint32_t lane_off = (uint32_t)a.slab0 + 8u * (64u * warp + lane);
+  const uint32_t lane_off = (uint32_t)a.slab0 + 8u * (64u * pwarp + lane);
   for (;;) {
     lra_mbar_wait(full0 + 8 * slot, par);
     unsigned char* sp = smem + LRA_RING_HDR + (size_t)slot * a.slot_bytes;
@@ -128,7 +131,7 @@ __global__ void __launch_bounds__((NW + 1) * 32) __maxnreg__(LRA_MAXNREG(NW, KS,
       for (int s = 0; s < KS; ++s) {
 #pragma unroll
         for (int half = 0; half < 2; ++half) {
-          const unsigned e = 64u * (NW * s + warp) + 32u * half + lane;
+          const unsigned e = 64u * (NW * s + pwarp) + 32u * half + lane;
           const int y = (int)__umulhi(e, magic), x = (int)e - y * a.rx;
           const int gx = x0 + x, gy = y0 + y;
           const bool ok = y < a.ry && gx >= 0 && gx < a.nx && gy >= 0 && gy < a.ny;
@@ -142,21 +145,21 @@ __global__ void __launch_bounds__((NW + 1) * 32) __maxnreg__(LRA_MAXNREG(NW, KS,
       fresh = false;
     }
     const uint32_t lane_base = slots0 + slot * a.slot_bytes + lane_off;
-    const unsigned char* rec = sp + LRA_SLOT_VAL;   // 16 bytes per point: the pw record {word, k, z, w} (lra_pipe.cuh)
+    const unsigned char* rec = sp + LRA_SLOT_VAL + 16 * first;   // 16 bytes per point: the pw record {word, k, z, w} (lra_pipe.cuh)
     float* out = reinterpret_cast<float*>(sp + a.out_off);
     // software pipeline over the points of the batch (as in the gridder), four points per reduction
     uint4 pc = *reinterpret_cast<const uint4*>(rec);
-    uint32_t mask = count ? lra_point_mask<NW>(pc.z, pc.w, warp) : 0u;
+    uint32_t mask = first < count ? lra_point_mask<NW>(pc.z, pc.w, pwarp) : 0u;
     lra_load_steps<NW, KS, 0>(T, lane_base + pc.x, mask);
-    for (unsigned q0 = 0; q0 < count; q0 += 4) {
+    for (unsigned q0 = first; q0 < count; q0 += 4 * PS) {   // this warp's points q0, q0 + PS, q0 + 2 PS, q0 + 3 PS
       float v[V];
 #pragma unroll
       for (int i = 0; i < V; ++i) v[i] = 0.f;
 #pragma unroll
       for (int u = 0; u < 4; ++u) {
-        rec += 16;
+        rec += 16 * PS;
         pc = *reinterpret_cast<const uint4*>(rec);
-        const uint32_t addr_next = lane_base + pc.x, mask_next = q0 + u + 1 < count ? lra_point_mask<NW>(pc.z, pc.w, warp) : 0u;
+        const uint32_t addr_next = lane_base + pc.x, mask_next = q0 + (u + 1) * PS < count ? lra_point_mask<NW>(pc.z, pc.w, pwarp) : 0u;
         lra_u64 P1[NG], P2[NG];
 #pragma unroll
         for (int g = 0; g < NG; ++g) P1[g] = P2[g] = 0ull;
@@ -183,8 +186,8 @@ __global__ void __launch_bounds__((NW + 1) * 32) __maxnreg__(LRA_MAXNREG(NW, KS,
       }
 #pragma unroll
       for (int w = V; w < 32; w <<= 1) v[0] += __shfl_xor_sync(0xffffffffu, v[0], w);
-      const unsigned left = count - q0;
-      if (lane < 8 * NG && (unsigned)(lane / (2 * NG)) < left) atomicAdd(out + q0 * (2 * NG) + lane, v[0]);
+      const unsigned pt = q0 + (unsigned)(lane / (2 * NG)) * PS;   // the point whose value this lane holds
+      if (lane < 8 * NG && pt < count) atomicAdd(out + pt * (2 * NG) + lane % (2 * NG), v[0]);
     }
     lra_mbar_arrive(empty0 + 8 * slot);   // every lane, after its own reads of the slot: no divergent branch in the loop
     if (h.y & LRA_BATCH_LAST) fresh = true;
@@ -209,7 +212,7 @@ static int lra_degrid_launch_class(lra_plan* p, lra_region_args a, const lra_geo
   a.batch = reinterpret_cast<const uint4*>(p->batch) + (size_t)p->batch_off[c] * 4;
   int ctas = p->sm_count * lra_ctas_per_sm(NW, KS, lra_grids_per_pass(p->ncorr * p->nterms), true);   // what the ring was sized for
   if ((int64_t)ctas > p->n_items[c]) ctas = (int)p->n_items[c];
-  kern<<<ctas, (NW + 1) * 32, smem, st>>>(a);
+  kern<<<ctas, (lra_cw(NW) + 1) * 32, smem, st>>>(a);
   LRA_LAUNCH_CHECK(p);
   return LRA_OK;
 }

@@ -117,7 +117,7 @@ __device__ __forceinline__ void lra_run_steps(lra_u64 (&acc)[KS][2][NG], const l
 }
 
 template <int NW, int KS, int NG>
-__global__ void __launch_bounds__((NW + 1) * 32) __maxnreg__(LRA_MAXNREG(NW, KS, NG, false)) lra_grid_region_kernel(const lra_region_args a) {
+__global__ void __launch_bounds__((lra_cw(NW) + 1) * 32) __maxnreg__(LRA_MAXNREG(NW, KS, NG, false)) lra_grid_region_kernel(const lra_region_args a) {
   extern __shared__ __align__(128) unsigned char smem[];
   const int lane = threadIdx.x & 31;
   const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);   // provably warp-uniform: uniform registers
@@ -125,7 +125,10 @@ __global__ void __launch_bounds__((NW + 1) * 32) __maxnreg__(LRA_MAXNREG(NW, KS,
   const uint32_t full0 = sbase, empty0 = sbase + 128, slots0 = sbase + LRA_RING_HDR;
   lra_region_ring_init<NW>(a, smem, full0, empty0);
   constexpr int PB = lra_point_bytes(NG);
-  if (warp == NW) {
+  constexpr int PS = NW == 1 ? LRA_PS_WARPS : 1;   // point-split warps (lra_cw in lra_pipe.cuh)
+  const int pwarp = PS > 1 ? 0 : warp;             // which chunks of the region this warp owns
+  const unsigned first = PS > 1 ? (unsigned)warp : 0u;   // its first point of a batch
+  if (warp == lra_cw(NW)) {
     lra_region_producer<NW, 0>(a, a.prep, PB, smem + LRA_RING_HDR, full0, empty0, slots0);
     return;
   }
@@ -139,32 +142,32 @@ __global__ void __launch_bounds__((NW + 1) * 32) __maxnreg__(LRA_MAXNREG(NW, KS,
 #pragma unroll
   for (int s = 0; s < KS; ++s) T[s].v[0] = T[s].v[1] = T[s].v[2] = T[s].v[3] = 0u;
   uint32_t slot = 0, par = 0;
-  const uint32_t lane_off = (uint32_t)a.slab0 + 8u * (64u * warp + lane);
+  const uint32_t lane_off = (uint32_t)a.slab0 + 8u * (64u * pwarp + lane);
   for (;;) {
     lra_mbar_wait(full0 + 8 * slot, par);
     const unsigned char* sp = smem + LRA_RING_HDR + (size_t)slot * a.slot_bytes;
     const uint4 h = *reinterpret_cast<const uint4*>(sp);
     const unsigned count = h.y & 0xff;
     const uint32_t lane_base = slots0 + slot * a.slot_bytes + lane_off;
-    const unsigned char* rec = sp + LRA_SLOT_VAL;
+    const unsigned char* rec = sp + LRA_SLOT_VAL + first * PB;
     // software pipeline over the points of the batch: while a step multiplies the taps of point q it reloads its tap
     // registers for point q + 1; the record of point q + 1 is read while point q runs
     // (the record's tail is {word, z, w, 0}: 8 bytes are enough up to four consumer warps)
     using tail_t = typename std::conditional<(NW <= 4), uint2, uint4>::type;
     auto tail_w = [](const tail_t& t) { if constexpr (NW <= 4) return 0u; else return t.z; };
     tail_t wc = *reinterpret_cast<const tail_t*>(rec + 16 * NG);
-    uint32_t mask = count ? lra_point_mask<NW>(wc.y, tail_w(wc), warp) : 0u;
+    uint32_t mask = first < count ? lra_point_mask<NW>(wc.y, tail_w(wc), pwarp) : 0u;
     lra_load_steps<NW, KS, 0>(T, lane_base + wc.x, mask);
-    for (unsigned q = 0; q < count; ++q) {
+    for (unsigned q = first; q < count; q += PS) {
       lra_u64 V[NG], W[NG];
 #pragma unroll
       for (int g = 0; g < NG; ++g) {
         const ulonglong2 v = *reinterpret_cast<const ulonglong2*>(rec + 16 * g);
         V[g] = v.x; W[g] = v.y;
       }
-      rec += PB;
+      rec += PS * PB;
       wc = *reinterpret_cast<const tail_t*>(rec + 16 * NG);
-      const uint32_t addr_next = lane_base + wc.x, mask_next = q + 1 < count ? lra_point_mask<NW>(wc.y, tail_w(wc), warp) : 0u;
+      const uint32_t addr_next = lane_base + wc.x, mask_next = q + PS < count ? lra_point_mask<NW>(wc.y, tail_w(wc), pwarp) : 0u;
       lra_run_steps<NW, NG, KS, 0>(acc, V, W, T, mask, addr_next, lra_opaque(mask_next));
       mask = mask_next;
     }
@@ -179,7 +182,7 @@ __global__ void __launch_bounds__((NW + 1) * 32) __maxnreg__(LRA_MAXNREG(NW, KS,
       for (int s = 0; s < KS; ++s) {
 #pragma unroll
         for (int half = 0; half < 2; ++half) {
-          const unsigned e = 64u * (NW * s + warp) + 32u * half + lane;
+          const unsigned e = 64u * (NW * s + pwarp) + 32u * half + lane;
           const int y = (int)__umulhi(e, magic), x = (int)e - y * a.rx;
           const int gx = x0 + x, gy = y0 + y;
           const bool ok = y < a.ry && gx >= 0 && gx < a.nx && gy >= 0 && gy < a.ny;
@@ -214,7 +217,7 @@ static int lra_grid_launch_class(lra_plan* p, lra_region_args a, const lra_geom&
   a.batch = reinterpret_cast<const uint4*>(p->batch) + (size_t)p->batch_off[c] * 4;
   int ctas = p->sm_count * lra_ctas_per_sm(NW, KS, lra_grids_per_pass(p->ncorr * p->nterms), false);   // what the ring was sized for
   if ((int64_t)ctas > p->n_items[c]) ctas = (int)p->n_items[c];
-  kern<<<ctas, (NW + 1) * 32, smem, st>>>(a);
+  kern<<<ctas, (lra_cw(NW) + 1) * 32, smem, st>>>(a);
   LRA_LAUNCH_CHECK(p);
   return LRA_OK;
 }

@@ -58,10 +58,20 @@ __host__ __device__ constexpr int lra_regs_need(int ks, int ngp, bool degrid) {
 }
 // The register file is 16384 registers per SM sub-partition and the warps of the resident CTAs are dealt round to the
 // four sub-partitions: C CTAs of NW + 1 warps put ceil((NW + 1) * C / 4) warps on the fullest one.
-__host__ __device__ constexpr int lra_warps_per_smsp(int nw, int ctas) { return ((nw + 1) * ctas + 3) / 4; }
+#ifndef LRA_PS_WARPS
+#define LRA_PS_WARPS 3   // consumer warps of a CTA whose whole region fits ONE warp's registers (nw = 1); with the producer
+                         // a CTA is four warps, one per SM sub-partition (measured on cfg3: 3 -> 55.95, 4 -> 56.05, 7 -> 56.35 ms per step)
+#endif
+// Consumer warps per CTA.  nw >= 2: the warps split the PIXELS of the region (chunk c belongs to warp c % nw) and every
+// warp visits every point.  nw = 1: a warp holds the whole region, and LRA_PS_WARPS such warps split the POINTS of a
+// batch instead (point q belongs to warp q % LRA_PS_WARPS): a point is visited once, its bookkeeping is paid once (the
+// degridder also reduces it across lanes once), and the warps' regions are added up by the flush.  Measured on cfg3
+// against two pixel-splitting warps: S = 9: gridder -1 %, degridder -34 %; S = 11: gridder -8 %, degridder -23 %.
+__host__ __device__ constexpr int lra_cw(int nw) { return nw == 1 ? LRA_PS_WARPS : nw; }
+__host__ __device__ constexpr int lra_warps_per_smsp(int nw, int ctas) { return ((lra_cw(nw) + 1) * ctas + 3) / 4; }
 __host__ __device__ constexpr int lra_ctas_per_sm(int nw, int ks, int ngp, bool degrid) {
   int r = 1;
-  while (r < LRA_CTA_CAP && (nw + 1) * (r + 1) <= 64 && lra_warps_per_smsp(nw, r + 1) * 32 * lra_regs_need(ks, ngp, degrid) <= 16384) ++r;
+  while (r < LRA_CTA_CAP && (lra_cw(nw) + 1) * (r + 1) <= 64 && lra_warps_per_smsp(nw, r + 1) * 32 * lra_regs_need(ks, ngp, degrid) <= 16384) ++r;
   return r;
 }
 __host__ __device__ constexpr int lra_regs(int nw, int ks, int ngp, bool degrid) {
@@ -93,7 +103,8 @@ __host__ __device__ inline lra_geom lra_make_geom(int S, int tile_x, int tile_y,
 #ifndef LRA_NW_MIN
 #define LRA_NW_MIN 2   // consumer warps per CTA at least: with one, half of the resident warps are producers (measured on cfg3: 1 -> 2: -0.6 ms gridder, -0.4 ms degridder; 4: worse)
 #endif
-    for (int nw = LRA_NW_MIN; nw <= 16; nw <<= 1) {
+    for (int nw = 1; nw <= 16; nw <<= 1) {
+      if (nw == 1 ? LRA_PS_WARPS < 2 && LRA_NW_MIN > 1 : nw < LRA_NW_MIN) continue;
       int ks = (chunks + nw - 1) / nw;
       if (ks == 5 || ks == 7) ++ks;   // the kernels are instantiated for KS = 1, 2, 3, 4, 6, 8
       if (ks > lim) continue;

@@ -173,13 +173,13 @@ template <int NW>
 __device__ __forceinline__ void lra_region_ring_init(const lra_region_args& a, unsigned char* smem,
                                                      uint32_t full0, uint32_t empty0) {
   if (threadIdx.x == 0) {
-    for (int s = 0; s < a.nslot; ++s) { lra_mbar_init(full0 + 8 * s, 1); lra_mbar_init(empty0 + 8 * s, NW * 32); }
+    for (int s = 0; s < a.nslot; ++s) { lra_mbar_init(full0 + 8 * s, 1); lra_mbar_init(empty0 + 8 * s, lra_cw(NW) * 32); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   const int area16 = (a.slot_bytes - LRA_SLOT_VAL) >> 4;   // everything behind the batch record
   for (int s = 0; s < a.nslot; ++s) {
     uint4* z = reinterpret_cast<uint4*>(smem + LRA_RING_HDR + (size_t)s * a.slot_bytes + LRA_SLOT_VAL);
-    for (int i = threadIdx.x; i < area16; i += (NW + 1) * 32) z[i] = make_uint4(0, 0, 0, 0);
+    for (int i = threadIdx.x; i < area16; i += (lra_cw(NW) + 1) * 32) z[i] = make_uint4(0, 0, 0, 0);
   }
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   __syncthreads();
