@@ -84,7 +84,10 @@ int lra_plan_destroy(lra_plan* p);
  *   cf_index    : device int32 [nrow][nchan] kernel of every point, or NULL (=> kernel 0)
  * The input arrays are not referenced after the call's stream work completes.
  * Synchronises the plan's stream ONCE, between its two passes over the sorted points (the host sizes the work lists of
- * lra_grid / lra_degrid from the per-class counts), and again whenever the plan's arrays have to grow.
+ * lra_grid / lra_degrid from the per-class counts), and again whenever the plan's arrays have to grow.  The few hundred
+ * bytes that cross the bus inside the call (the per-channel scales, the list sizes) go through kernels on pinned, mapped
+ * memory, not through cudaMemcpy, so the call does not queue behind bulk transfers the caller has in flight on other
+ * streams.
  * Errors: LRA_EINVAL, LRA_ENOMEM (growing the plan's bin arrays), LRA_ECUDA. */
 int lra_bin(lra_plan* p, int64_t nrow, int32_t nchan, const double* uvw_m, const double* freq_hz,
             const int32_t* cf_index);

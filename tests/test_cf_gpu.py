@@ -155,6 +155,21 @@ def test_generated_table_feeds_the_plan_from_device_memory(B, ref):
     np.testing.assert_allclose(sw.cpu().numpy(), want_sw, rtol=1e-6)
 
 
+def test_cf_generate_extreme_shapes(B, ref):
+    """No oversampling, the smallest and the largest support, an odd raster, a raster smaller than the support."""
+    for n, os_, sup in ((33, 1, [1, 3, 129]), (140, 2, [129]), (8, 4, [31])):
+        taper, aterm = _inputs(n, 1, n + os_)
+        w = np.linspace(-50.0, 900.0, len(sup))
+        off, total = _offsets(sup, os_)
+        out = torch.zeros(total, dtype=torch.complex64, device="cuda")
+        B.lra_cf_generate(out, n, os_, 0.04, sup, off, taper=dev(taper), aterm=dev(aterm), cf_w=w)
+        got = out.cpu().numpy()
+        for c, S in enumerate(sup):
+            so = S * os_
+            want = ref.cf(n, os_, 0.04, S, taper=taper, w_lambda=float(w[c]), aterm=aterm[0].astype(np.complex128))
+            _assert_cf_close(got[off[c]: off[c] + so * so].reshape(so, so), want, f"n={n} os={os_} S={S}")
+
+
 def test_cf_generate_errors(B):
     out = torch.zeros(4096, dtype=torch.complex64, device="cuda")
     t = torch.ones(16, dtype=torch.float64, device="cuda")
