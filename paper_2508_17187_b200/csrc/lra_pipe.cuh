@@ -180,6 +180,10 @@ __device__ __forceinline__ void lra_mbar_init(uint32_t bar, uint32_t count) {
 __device__ __forceinline__ void lra_mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
+// Adds to the transaction count only: the phase still needs the arrival (lra_mbar_arrive), which may come later.
+__device__ __forceinline__ void lra_mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.expect_tx.relaxed.cta.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
 __device__ __forceinline__ void lra_mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }

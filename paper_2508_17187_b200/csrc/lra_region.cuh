@@ -37,9 +37,8 @@ __device__ __forceinline__ void lra_region_producer(const lra_region_args& a, co
   const int lane = threadIdx.x & 31;
   const uint32_t slab0 = (uint32_t)a.slab0;
   uint32_t slot = 0, par = 0, issued = 0;
-  auto write_out = [&](uint32_t s) {   // all lanes; every consumer warp has released slot s
+  auto write_out_h = [&](uint32_t s, const uint4 h) {   // all lanes; every consumer warp has released slot s; h: its header
     unsigned char* sp = slots + (size_t)s * a.slot_bytes;
-    const uint4 h = *reinterpret_cast<const uint4*>(sp);
     const unsigned cnt = (h.y & 0xff) * OUTW;
     float2* out = reinterpret_cast<float2*>(sp + a.out_off);
     for (unsigned i = lane; i < cnt; i += 32) {
@@ -47,6 +46,7 @@ __device__ __forceinline__ void lra_region_producer(const lra_region_args& a, co
       out[i] = make_float2(0.f, 0.f);
     }
   };
+  auto write_out = [&](uint32_t s) { write_out_h(s, *reinterpret_cast<const uint4*>(slots + (size_t)s * a.slot_bytes)); };
   // tickets and item records are fetched one item ahead, batch records eight batches ahead: lane l of a group of
   // eight batches holds quarter l % 4 of the record of batch l / 4
   unsigned long long t_nxt = 0;
@@ -72,10 +72,15 @@ __device__ __forceinline__ void lra_region_producer(const lra_region_args& a, co
         // lane 4j owns the batch: slot hand-over, record, prepared values
         const uint32_t sa = slots0 + slot * a.slot_bytes, fb = full0 + 8 * slot;
         const uint32_t nr = __shfl_sync(0xffffffffu, cur.z, 4 * j) & 0xff;
+        // degridder: the results the slot's previous batch left are written out AFTER the copies of the new batch have
+        // been issued (they touch other parts of the slot), so the write-out hides behind the copies' latency instead
+        // of delaying them; the barrier's arrival, which the consumers wait for besides the bytes, comes last
+        uint4 h_old = make_uint4(0u, 0u, 0u, 0u);
+        const bool had = OUTW > 0 && issued >= (uint32_t)a.nslot;
         if (OUTW > 0) {
           if (lane == 0) lra_mbar_wait(empty0 + 8 * slot, par ^ 1);
           __syncwarp();
-          if (issued >= (uint32_t)a.nslot) write_out(slot);
+          if (had) h_old = *reinterpret_cast<const uint4*>(slots + (size_t)slot * a.slot_bytes);
           __syncwarp();
         }
         ++issued;
@@ -84,7 +89,9 @@ __device__ __forceinline__ void lra_region_producer(const lra_region_args& a, co
           const bool pv = vals != nullptr;
           lra_mbar_wait(empty0 + 8 * slot, par ^ 1);
           asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(sa), "r"(cur.x), "r"(cur.y), "r"(cur.z), "r"(cur.w) : "memory");
-          lra_mbar_arrive_expect_tx(fb, (pv ? count * val_bytes : 0u) + nr * (uint32_t)a.core_bytes);
+          const uint32_t bytes = (pv ? count * val_bytes : 0u) + nr * (uint32_t)a.core_bytes;
+          if (OUTW > 0) lra_mbar_expect_tx(fb, bytes);
+          else lra_mbar_arrive_expect_tx(fb, bytes);
           if (pv) lra_tma_load_1d(sa + LRA_SLOT_VAL, reinterpret_cast<const unsigned char*>(vals) + (size_t)cur.x * val_bytes, count * val_bytes, fb);
         }
         __syncwarp();   // the slot is free from here on
@@ -98,6 +105,11 @@ __device__ __forceinline__ void lra_region_producer(const lra_region_args& a, co
             const unsigned char* src_b = reinterpret_cast<const unsigned char*>(a.slabs) + ((size_t)off16 << 4);
             lra_tma_load_1d(sa + slab0 + a.gap_bytes + r * a.stride_bytes, src_b, a.core_bytes, fb);
           }
+        }
+        if (OUTW > 0) {
+          if (had) write_out_h(slot, h_old);
+          __syncwarp();
+          if (lane == (int)(4 * j)) lra_mbar_arrive(fb);
         }
         if (++slot == (uint32_t)a.nslot) { slot = 0; par ^= 1; }
       }
