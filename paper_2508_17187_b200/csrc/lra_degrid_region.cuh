@@ -151,6 +151,9 @@ __global__ void __launch_bounds__((lra_cw(NW) + 1) * 32) __maxnreg__(LRA_MAXNREG
     uint4 pc = *reinterpret_cast<const uint4*>(rec);
     uint32_t mask = first < count ? lra_point_mask<NW>(pc.z, pc.w, pwarp) : 0u;
     lra_load_steps<NW, KS, 0>(T, lane_base + pc.x, mask);
+    // Two releases per slot: its taps and records once this warp has loaded the last of them (the producer may then start
+    // the copies of the slot's next batch), its results at the end of the batch.
+    if (first >= count) lra_mbar_arrive(empty0 + 8 * slot);
     for (unsigned q0 = first; q0 < count; q0 += 4 * PS) {   // this warp's points q0, q0 + PS, q0 + 2 PS, q0 + 3 PS
       float v[V];
 #pragma unroll
@@ -160,6 +163,9 @@ __global__ void __launch_bounds__((lra_cw(NW) + 1) * 32) __maxnreg__(LRA_MAXNREG
         rec += 16 * PS;
         pc = *reinterpret_cast<const uint4*>(rec);
         const uint32_t addr_next = lane_base + pc.x, mask_next = q0 + (u + 1) * PS < count ? lra_point_mask<NW>(pc.z, pc.w, pwarp) : 0u;
+        // the warp's last point of the batch: its taps were loaded during the point before (the arrival is ordered
+        // after those loads), nothing of the slot but the result area is touched from here on
+        if (q0 + u * PS < count && q0 + (u + 1) * PS >= count) lra_mbar_arrive(empty0 + 8 * slot);
         lra_u64 P1[NG], P2[NG];
 #pragma unroll
         for (int g = 0; g < NG; ++g) P1[g] = P2[g] = 0ull;
@@ -189,7 +195,7 @@ __global__ void __launch_bounds__((lra_cw(NW) + 1) * 32) __maxnreg__(LRA_MAXNREG
       const unsigned pt = q0 + (unsigned)(lane / (2 * NG)) * PS;   // the point whose value this lane holds
       if (lane < 8 * NG && pt < count) atomicAdd(out + pt * (2 * NG) + lane % (2 * NG), v[0]);
     }
-    lra_mbar_arrive(empty0 + 8 * slot);   // every lane, after its own reads of the slot: no divergent branch in the loop
+    lra_mbar_arrive(empty0 + LRA_EMPTY_OUT + 8 * slot);   // every lane (no divergent branch in the loop): the results are complete
     if (h.y & LRA_BATCH_LAST) fresh = true;
     if (h.y & LRA_BATCH_END) break;
     if (++slot == (uint32_t)a.nslot) { slot = 0; par ^= 1; }

@@ -25,7 +25,8 @@ struct lra_region_args {
 // gap, slab of run 1, ...: the kernel zeroes it once and the copies only ever write the slabs, so the gaps stay
 // zero for the whole launch (one launch = one support class = one geometry).
 #define LRA_SLOT_VAL 128
-#define LRA_RING_HDR 256   // full / empty barriers of up to 16 slots
+#define LRA_RING_HDR 256   // full barriers at +0, empty barriers at +128, the degridder's second empty set at +192 (<= 4 slots)
+#define LRA_EMPTY_OUT 64   // offset of that second set from the first: "the results of the slot may be written out"
 
 // Producer warp, shared by the gridder and the degridder: walks the items (atomic ticket) and their batches and
 // fills the ring: batch record, `val_bytes` per point from `vals` (if any) and the slab planes.  OUTW > 0 (degridder):
@@ -107,7 +108,11 @@ __device__ __forceinline__ void lra_region_producer(const lra_region_args& a, co
           }
         }
         if (OUTW > 0) {
-          if (had) write_out_h(slot, h_old);
+          if (had) {   // the consumers release the slot's results later than its taps (lra_degrid_region.cuh)
+            if (lane == 0) lra_mbar_wait(empty0 + LRA_EMPTY_OUT + 8 * slot, par ^ 1);
+            __syncwarp();
+            write_out_h(slot, h_old);
+          }
           __syncwarp();
           if (lane == (int)(4 * j)) lra_mbar_arrive(fb);
         }
@@ -120,7 +125,7 @@ __device__ __forceinline__ void lra_region_producer(const lra_region_args& a, co
       uint32_t s = slot + u, p = par ^ 1;
       if (s >= (uint32_t)a.nslot) { s -= a.nslot; p = par; }
       if (s >= issued) continue;
-      if (lane == 0) lra_mbar_wait(empty0 + 8 * s, p);
+      if (lane == 0) lra_mbar_wait(empty0 + LRA_EMPTY_OUT + 8 * s, p);
       __syncwarp();
       write_out(s);
       __syncwarp();
@@ -185,7 +190,11 @@ template <int NW>
 __device__ __forceinline__ void lra_region_ring_init(const lra_region_args& a, unsigned char* smem,
                                                      uint32_t full0, uint32_t empty0) {
   if (threadIdx.x == 0) {
-    for (int s = 0; s < a.nslot; ++s) { lra_mbar_init(full0 + 8 * s, 1); lra_mbar_init(empty0 + 8 * s, lra_cw(NW) * 32); }
+    for (int s = 0; s < a.nslot; ++s) {
+      lra_mbar_init(full0 + 8 * s, 1);
+      lra_mbar_init(empty0 + 8 * s, lra_cw(NW) * 32);
+      lra_mbar_init(empty0 + LRA_EMPTY_OUT + 8 * s, lra_cw(NW) * 32);
+    }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   const int area16 = (a.slot_bytes - LRA_SLOT_VAL) >> 4;   // everything behind the batch record
