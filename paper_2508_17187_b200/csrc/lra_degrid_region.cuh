@@ -233,6 +233,7 @@ static int lra_degrid_launch_ks(lra_plan* p, const lra_region_args& a, const lra
     default: break;
   }
   if constexpr (NG <= 2) {
+    if (q.ks == 5) return lra_degrid_launch_class<NW, 5, NG>(p, a, q, c, st);
     if (q.ks == 6) return lra_degrid_launch_class<NW, 6, NG>(p, a, q, c, st);
   }
   if constexpr (NG == 1) {

@@ -106,7 +106,7 @@ __host__ __device__ inline lra_geom lra_make_geom(int S, int tile_x, int tile_y,
     for (int nw = 1; nw <= 16; nw <<= 1) {
       if (nw == 1 ? LRA_PS_WARPS < 2 && LRA_NW_MIN > 1 : nw < LRA_NW_MIN) continue;
       int ks = (chunks + nw - 1) / nw;
-      if (ks == 5 || ks == 7) ++ks;   // the kernels are instantiated for KS = 1, 2, 3, 4, 6, 8
+      if (ks == 7 || (ks == 5 && ngp > 2)) ++ks;   // the kernels are instantiated for KS = 1, 2, 3, 4, 5 (one or two grids), 6, 8
       if (ks > lim) continue;
       q.nw = nw; q.ks = ks;
       break;
