@@ -229,6 +229,28 @@ int lra_grid_po(lra_plan* p, const void* vis_c64, const float* wt, const float* 
 int lra_degrid_po(lra_plan* p, const void* grid_c64, const float* tau, int32_t n_po, const double* po_table,
                   const int32_t* po_index, const void* vis_in_c64, void* vis_out_c64);
 
+/* lra_phase_gradient for callers that must not allocate (CUDA graph capture, serving loops, harnesses that forbid
+ * cudaMalloc).  The operation is lra_phase_gradient's (the pointing factor of Eq. 27, reading R27):
+ *   dst[g][Y][X] (+)= f e^{+-2 pi i (dl (X - nx/2)/scale_u + dm (Y - ny/2)/scale_v)} src[g][Y][X],  g < nplanes,
+ * "-" with conjugate != 0, "+=" with accumulate != 0; src == dst allowed without accumulate.  It takes no plan: the
+ * geometry is passed in, the CURRENT device is used and the two kernels are enqueued on `stream` (a cudaStream_t; NULL =
+ * the default stream); the call returns without synchronising.
+ *   src, dst : DEVICE complex64 [nplanes][ny][nx], caller-owned;  scale_u, scale_v : pixels per wavelength, non-zero.
+ * Scratch: the nx + ny phasors the kernels share live in a file-scope device array of LRA_STATIC_MAX_AXES complex64
+ * (512 KiB, held by every GPU that loads the library until the process exits).  The call issues no cudaMalloc, cudaFree or
+ * allocating library call; the first call on a device resolves the array's address (cudaGetSymbolAddress) and reads the
+ * SM count, so make one call per device before capturing a graph.  Every call on a device uses the SAME array and
+ * rewrites the entries it reads (nothing needs clearing): calls whose kernels overlap on the GPU (different streams
+ * without a dependency between them, or concurrent host threads on different streams) race -- order them on one stream or
+ * with events.
+ * Errors: LRA_EINVAL (NULL src / dst, nx, ny or nplanes < 1, nx + ny > LRA_STATIC_MAX_AXES, NaN factor, zero scale),
+ * LRA_ECUDA; lra_static_last_error() returns a description of this thread's last failure ("" after a success). */
+#define LRA_STATIC_MAX_AXES 65536
+int lra_phase_gradient_static(int32_t nx, int32_t ny, int32_t nplanes, double scale_u, double scale_v, const void* src_c64,
+                              double f, double dl, double dm, int32_t conjugate, int32_t accumulate, void* dst_c64,
+                              void* stream);
+const char* lra_static_last_error(void);
+
 /* Sparse Mueller matrix of CFs: element e = (grid plane elem_grid[e], visibility correlation elem_corr[e])
  * has its own kernel index per visibility point, cf_index[e] (HOST array of n_elem DEVICE pointers to int32 [nrow][nchan],
  * NULL entry = kernel 0).  Gridding adds CF_e (x) [wt V]_{elem_corr[e]} to plane elem_grid[e]; degridding subtracts (adds,

@@ -17,6 +17,7 @@ from . import _build
 
 LRA_OK, LRA_EINVAL, LRA_ENOMEM, LRA_ECUDA, LRA_ESTATE = 0, 1, 2, 3, 4
 LRA_SORT_TILE, LRA_SORT_TILE_CF = 0, 1
+LRA_STATIC_MAX_AXES = 65536   # lra.h: largest nx + ny lra_phase_gradient_static accepts
 
 
 class LraError(RuntimeError):
@@ -64,6 +65,9 @@ def lib() -> C.CDLL:
         L.lra_gain_solve.argtypes = [i32, vp, i32, i32, i32, vp, vp, vp, vp, C.c_double, C.c_double, i32, vp, vp]
         L.lra_cf_generate.argtypes = [C.POINTER(lra_cf_desc), vp]
         L.lra_phase_gradient.argtypes = [vp, vp, C.c_double, C.c_double, C.c_double, i32, i32, vp]
+        L.lra_phase_gradient_static.argtypes = [i32, i32, i32, C.c_double, C.c_double, vp, C.c_double, C.c_double, C.c_double,
+                                                i32, i32, vp, vp]
+        L.lra_static_last_error.restype = C.c_char_p
         L.lra_grid_po.argtypes = [vp, vp, vp, vp, i32, vp, vp, vp, vp]
         L.lra_degrid_po.argtypes = [vp, vp, vp, i32, vp, vp, vp, vp]
         L.lra_grid_mueller.argtypes = [vp, i64, i32, vp, vp, i32, vp, vp, vp, i32, vp, vp, vp, i32, vp, vp, i32, vp, vp]
@@ -85,7 +89,7 @@ def lib() -> C.CDLL:
 
 EXPORTED = ["lra_plan_create", "lra_plan_destroy", "lra_bin", "lra_bin_export", "lra_grid", "lra_degrid", "lra_image",
             "lra_model_grid", "lra_gain_accumulate", "lra_gain_solve", "lra_cf_generate", "lra_cf_last_cuda_error",
-            "lra_phase_gradient", "lra_grid_po", "lra_degrid_po", "lra_grid_mueller", "lra_degrid_mueller",
+            "lra_phase_gradient", "lra_phase_gradient_static", "lra_static_last_error", "lra_grid_po", "lra_degrid_po", "lra_grid_mueller", "lra_degrid_mueller",
             "lra_launch_count", "lra_tap_count", "lra_set_variant", "lra_strerror", "lra_last_cuda_error",
             "lra_diag_fma_tflops", "lra_diag_l2_gbs"]
 
@@ -265,6 +269,29 @@ def lra_phase_gradient(plan: int, src, f, dl, dm, dst, conjugate=False, accumula
         raise LraError("src and dst must have the same shape")
     _check(lib().lra_phase_gradient(plan, _dev(src, torch.complex64, plan), float(f), float(dl), float(dm),
                                     1 if conjugate else 0, 1 if accumulate else 0, _dev(dst, torch.complex64, plan)), plan)
+
+
+def lra_phase_gradient_static(src, scale_u, scale_v, f, dl, dm, dst, conjugate=False, accumulate=False, stream=None):
+    """lra_phase_gradient without a plan and without any allocation (lra.h: lra_phase_gradient_static): src, dst CUDA
+    complex64 [..., ny, nx] on the current device; enqueued on `stream` (a torch.cuda.Stream; default: the current one)."""
+    import torch
+    if src.shape != dst.shape or src.dim() < 2:
+        raise LraError("src and dst must have the same shape [..., ny, nx]")
+    if src.device != dst.device or src.device.index != torch.cuda.current_device():
+        raise LraError("src and dst must live on the current CUDA device")
+    ny, nx = int(src.shape[-2]), int(src.shape[-1])
+    nplanes = int(src.numel() // (nx * ny)) if nx * ny else 0
+    s = stream if stream is not None else torch.cuda.current_stream()
+    rc = lib().lra_phase_gradient_static(nx, ny, nplanes, float(scale_u), float(scale_v), _dev(src, torch.complex64), float(f),
+                                         float(dl), float(dm), 1 if conjugate else 0, 1 if accumulate else 0,
+                                         _dev(dst, torch.complex64), s.cuda_stream)
+    if rc != LRA_OK:
+        raise LraError(f"liblra: {lib().lra_strerror(rc).decode()} ({lra_static_last_error()}) [code {rc}]")
+
+
+def lra_static_last_error() -> str:
+    """Description of this thread's last lra_phase_gradient_static failure ("" after a success)."""
+    return lib().lra_static_last_error().decode()
 
 
 def lra_grid_po(plan: int, vis, wt, tau, po_table, po_index, grid, sumwt=None):

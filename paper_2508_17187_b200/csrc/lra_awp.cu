@@ -13,6 +13,9 @@
 // element's visibility correlation, grid onto / degrid from the element's grid plane.
 // Product code: shares nothing with oracle/.
 #include <algorithm>
+#include <cstdarg>
+#include <cstdio>
+#include <mutex>
 
 #include "lra_pipe.cuh"
 
@@ -446,3 +449,86 @@ extern "C" int lra_degrid_mueller(lra_plan* p, int64_t nrow, int32_t nchan, cons
   cudaFree(v1);
   return rc;
 }
+
+// ---- lra_phase_gradient_static: the phase gradient for callers that must not allocate -----------------------------------
+// Same two kernels as lra_phase_gradient; the phasor table tab[nx + ny] lives in a file-scope device array instead of the
+// plan's awp_buf, so the call needs no plan and issues no cudaMalloc / cudaFree (graph capture, serving loops).  Every
+// GPU that loads liblra.so holds LRA_STATIC_MAX_AXES * 8 bytes = 512 KiB for it until the process exits.  The array is
+// shared by all calls on a device: each call rewrites entries [0, nx + ny) before it reads them (nothing has to start at
+// zero), and two calls whose kernels overlap on the GPU (different streams, no dependency) race on it.
+static __device__ __align__(256) float2 lra_static_tab[LRA_STATIC_MAX_AXES];
+
+namespace {
+
+constexpr int LRA_STATIC_MAX_DEVICES = 64;
+struct lra_static_device { float2* tab; int sm_count; };
+lra_static_device lra_static_dev[LRA_STATIC_MAX_DEVICES];   // tab == nullptr: not resolved yet
+std::mutex lra_static_mutex;
+thread_local char lra_static_error[256] = "";
+
+int lra_static_fail(int code, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(lra_static_error, sizeof(lra_static_error), fmt, ap);
+  va_end(ap);
+  return code;
+}
+
+// In host code `lra_static_tab` is a host-side handle, not a device address: resolve it once per device, with that device
+// current, and hand the resolved pointer to the kernels.
+int lra_static_resolve(int device, lra_static_device* out) {
+  std::lock_guard<std::mutex> lock(lra_static_mutex);
+  lra_static_device& d = lra_static_dev[device];
+  if (!d.tab) {
+    float2* ptr = nullptr;
+    cudaError_t e = cudaGetSymbolAddress((void**)&ptr, lra_static_tab);
+    if (e != cudaSuccess || !ptr)
+      return lra_static_fail(LRA_ECUDA, "cudaGetSymbolAddress(lra_static_tab) on device %d: %s", device, cudaGetErrorString(e));
+    int sms = 0;
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
+    if (e != cudaSuccess || sms < 1)
+      return lra_static_fail(LRA_ECUDA, "cudaDeviceGetAttribute(sm count) on device %d: %s", device, cudaGetErrorString(e));
+    d.sm_count = sms;
+    d.tab = ptr;
+  }
+  *out = d;
+  return LRA_OK;
+}
+
+}  // namespace
+
+extern "C" int lra_phase_gradient_static(int32_t nx, int32_t ny, int32_t nplanes, double scale_u, double scale_v,
+                                         const void* src, double f, double dl, double dm, int32_t conjugate,
+                                         int32_t accumulate, void* dst, void* stream) {
+  lra_static_error[0] = 0;
+  if (!src || !dst) return lra_static_fail(LRA_EINVAL, "lra_phase_gradient_static: src and dst must not be NULL");
+  if (nx < 1 || ny < 1 || nplanes < 1)
+    return lra_static_fail(LRA_EINVAL, "lra_phase_gradient_static: nx = %d, ny = %d, nplanes = %d must be >= 1", nx, ny, nplanes);
+  if ((long long)nx + ny > LRA_STATIC_MAX_AXES)
+    return lra_static_fail(LRA_EINVAL, "lra_phase_gradient_static: nx + ny = %lld exceeds the static table of LRA_STATIC_MAX_AXES = %d "
+                           "entries; use lra_phase_gradient (plan-owned scratch) for larger grids", (long long)nx + ny, LRA_STATIC_MAX_AXES);
+  if (!(f == f) || !(dl == dl) || !(dm == dm) || !(scale_u == scale_u) || !(scale_v == scale_v) || scale_u == 0.0 || scale_v == 0.0)
+    return lra_static_fail(LRA_EINVAL, "lra_phase_gradient_static: f, dl, dm must be numbers and scale_u, scale_v non-zero");
+  int device = -1;
+  cudaError_t e = cudaGetDevice(&device);
+  if (e != cudaSuccess) return lra_static_fail(LRA_ECUDA, "cudaGetDevice: %s", cudaGetErrorString(e));
+  if (device < 0 || device >= LRA_STATIC_MAX_DEVICES)
+    return lra_static_fail(LRA_EINVAL, "lra_phase_gradient_static: device ordinal %d not below %d", device, LRA_STATIC_MAX_DEVICES);
+  lra_static_device d;
+  int rc = lra_static_resolve(device, &d);
+  if (rc != LRA_OK) return rc;
+  cudaStream_t s = (cudaStream_t)stream;
+  const double sgn = conjugate ? -1.0 : 1.0;
+  lra_gradient_table_kernel<<<(nx + ny + 255) / 256, 256, 0, s>>>(d.tab, nx, ny, sgn * dl / scale_u, sgn * dm / scale_v, f);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return lra_static_fail(LRA_ECUDA, "lra_gradient_table_kernel launch: %s", cudaGetErrorString(e));
+  const long long n = (long long)nplanes * nx * ny;
+  const int blocks = (int)std::min<long long>((n + 255) / 256, (long long)d.sm_count * 16);
+  if (accumulate) lra_phase_gradient_kernel<true><<<blocks, 256, 0, s>>>((const float2*)src, d.tab, (float2*)dst, nx, ny, n);
+  else lra_phase_gradient_kernel<false><<<blocks, 256, 0, s>>>((const float2*)src, d.tab, (float2*)dst, nx, ny, n);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return lra_static_fail(LRA_ECUDA, "lra_phase_gradient_kernel launch: %s", cudaGetErrorString(e));
+  return LRA_OK;
+}
+
+extern "C" const char* lra_static_last_error(void) { return lra_static_error; }
