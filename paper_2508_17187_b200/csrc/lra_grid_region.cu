@@ -13,40 +13,50 @@ int lra_grid_launch_ng(lra_plan* p, const lra_region_args& a, const lra_geom& q,
 // with word and the step masks / chunk range (z, w) from lra_work.cu (lra_pipe.cuh).  Every pass but the last holds LRA_NGMAX grids, so
 // pass j starts npoints * j * lra_point_bytes(LRA_NGMAX) bytes into `prep`.  One thread per point; the same pass over
 // the weights also gives sumwt[t][p] += wt*tau (fp64 partials per thread, block tree, one atomic per block and grid).
-__global__ void __launch_bounds__(256)
+// NCORR, NTERMS > 0: sizes known at compile time (the common shapes: the fp64 sumwt partials then take NCORR * NTERMS
+// register pairs instead of 16: 48 instead of 140 registers); NCORR = 0: any shape up to 4 x 4.
+// Launched with ONE block of 256 threads per SM: the pass is a random gather (16 + 8 useful bytes per point out of two
+// 64-byte DRAM bursts) and runs fastest with 256-512 gathers in flight per SM -- measured on cfg3, whole lra_grid call:
+// 1 x 256 threads per SM 20.22 ms, 2 x 256 20.53, 4 x 256 20.63, 8 x 256 (full occupancy) 20.85, 1 x 128 20.78,
+// 1 x 512 20.42, 1 x 1024 20.57; two or four points per thread in flight: 20.24 / 20.41.
+#define LRA_PREP_THREADS 256
+template <int NCORR, int NTERMS>
+__global__ void __launch_bounds__(LRA_PREP_THREADS)
 lra_prepare_kernel(const unsigned long long* __restrict__ counters, const uint4* __restrict__ pw,
                    const float2* __restrict__ vis, const float* __restrict__ wt, const float* __restrict__ tau,
-                   int nchan, int ncorr, int nterms, long long npoints, unsigned char* __restrict__ prep,
+                   int nchan, int ncorr_rt, int nterms_rt, long long npoints, unsigned char* __restrict__ prep,
                    double* __restrict__ sumwt, int fast2) {
   const long long n = (long long)counters[0];
+  const int ncorr = NCORR ? NCORR : ncorr_rt, nterms = NCORR ? NTERMS : nterms_rt;
+  constexpr int MC = NCORR ? NCORR : 4, MT = NCORR ? NTERMS : 4;
   const int ng = ncorr * nterms;
-  double acc[16];
+  double acc[MT * MC];
 #pragma unroll
-  for (int g = 0; g < 16; ++g) acc[g] = 0.0;
+  for (int g = 0; g < MT * MC; ++g) acc[g] = 0.0;
   for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
     const uint4 w4 = pw[i];
     const unsigned k = w4.y & 0x7fffffffu;
     const int c = (int)(k % (unsigned)nchan);
-    float2 v[4];
-    float w[4];
-    if (fast2) {   // two correlations, 16-byte aligned vis: one load each
+    float2 v[MC];
+    float w[MC];
+    if (MC == 2 && fast2) {   // two correlations, 16-byte aligned vis: one load each
       const float4 vv = *reinterpret_cast<const float4*>(vis + (size_t)k * 2);
       const float2 ww = *reinterpret_cast<const float2*>(wt + (size_t)k * 2);
       v[0] = make_float2(vv.x, vv.y); v[1] = make_float2(vv.z, vv.w); w[0] = ww.x; w[1] = ww.y;
     } else {
 #pragma unroll
-      for (int p = 0; p < 4; ++p)
+      for (int p = 0; p < MC; ++p)
         if (p < ncorr) { v[p] = vis[(size_t)k * ncorr + p]; w[p] = wt[(size_t)k * ncorr + p]; }
     }
 #pragma unroll
-    for (int t = 0; t < 4; ++t) {
+    for (int t = 0; t < MT; ++t) {
       if (t >= nterms) break;
       const float tw = tau ? tau[c * nterms + t] : 1.0f;
 #pragma unroll
-      for (int p = 0; p < 4; ++p) {
+      for (int p = 0; p < MC; ++p) {
         if (p >= ncorr) break;
         const float wgt = w[p] * tw;
-        acc[t * 4 + p] += (double)wgt;
+        acc[t * MC + p] += (double)wgt;
         const float vx = wgt * v[p].x, vy = wgt * v[p].y;
         const int g = t * ncorr + p, pass = g / LRA_NGMAX, gl = g - pass * LRA_NGMAX;
         const int ngp = ng - pass * LRA_NGMAX >= LRA_NGMAX ? LRA_NGMAX : ng - pass * LRA_NGMAX;
@@ -57,20 +67,20 @@ lra_prepare_kernel(const unsigned long long* __restrict__ counters, const uint4*
     }
   }
   if (!sumwt) return;
-  __shared__ double sh[8][16];
+  __shared__ double sh[LRA_PREP_THREADS / 32][MT * MC];
   const int l = threadIdx.x & 31, wp = threadIdx.x >> 5;
 #pragma unroll
-  for (int g = 0; g < 16; ++g) {
+  for (int g = 0; g < MT * MC; ++g) {
     double x = acc[g];
     for (int o = 16; o > 0; o >>= 1) x += __shfl_down_sync(0xffffffffu, x, o);
     if (l == 0) sh[wp][g] = x;
   }
   __syncthreads();
-  if (threadIdx.x < 16) {
-    const int t = threadIdx.x >> 2, pp = threadIdx.x & 3;
+  if (threadIdx.x < MT * MC) {
+    const int t = threadIdx.x / MC, pp = threadIdx.x % MC;
     if (t < nterms && pp < ncorr) {
       double x = 0.0;
-      for (int ww = 0; ww < 8; ++ww) x += sh[ww][threadIdx.x];
+      for (int ww = 0; ww < (int)(blockDim.x >> 5); ++ww) x += sh[ww][threadIdx.x];
       atomicAdd(&sumwt[t * ncorr + pp], x);
     }
   }
@@ -89,9 +99,18 @@ int lra_grid_region_launch(lra_plan* p, const float2* vis, const float* wt, cons
     LRA_CUDA(p, cudaMalloc(&p->prep, (size_t)need * sizeof(float)));
     p->prep_capacity = need;
   }
-  lra_prepare_kernel<<<p->sm_count * 8, 256, 0, p->stream>>>(p->counters, p->pw, vis, wt, tau, p->nchan, p->ncorr, p->nterms,
-                                                            (long long)n, reinterpret_cast<unsigned char*>(p->prep), sumwt,
-                                                            p->ncorr == 2 && ((uintptr_t)vis & 15) == 0 && ((uintptr_t)wt & 7) == 0);
+  {
+    const int fast2 = p->ncorr == 2 && ((uintptr_t)vis & 15) == 0 && ((uintptr_t)wt & 7) == 0;
+    unsigned char* prep = reinterpret_cast<unsigned char*>(p->prep);
+#define LRA_PREPARE(NC, NT) lra_prepare_kernel<NC, NT><<<p->sm_count, LRA_PREP_THREADS, 0, p->stream>>>(p->counters, p->pw, vis, wt, tau, \
+                                p->nchan, p->ncorr, p->nterms, (long long)n, prep, sumwt, fast2)
+    if (p->ncorr == 2 && p->nterms == 1) LRA_PREPARE(2, 1);
+    else if (p->ncorr == 2 && p->nterms == 2) LRA_PREPARE(2, 2);
+    else if (p->ncorr == 4 && p->nterms == 1) LRA_PREPARE(4, 1);
+    else if (p->ncorr == 1 && p->nterms == 1) LRA_PREPARE(1, 1);
+    else LRA_PREPARE(0, 0);
+#undef LRA_PREPARE
+  }
   LRA_LAUNCH_CHECK(p);
   LRA_CUDA(p, cudaMemsetAsync(p->counters + LRA_TICKET0, 0, LRA_NTICKET * sizeof(unsigned long long), p->stream));
   lra_region_args a;
