@@ -49,7 +49,7 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--grid-variant", type=int, default=0)
-    ap.add_argument("--tile", type=int, default=0, help="uv-tile height (0 = the config's, i.e. the library default)")
+    ap.add_argument("--tile", type=int, default=0, help="uv-tile height (0 = the config's: workloads.full_config)")
     ap.add_argument("--tile-x", type=int, default=0, help="uv-tile width (with --tile)")
     return ap.parse_args()
 
@@ -392,7 +392,7 @@ def run_ours(args):
                 "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
                 "data": "synthetic",
                 "config": {"workload": cfg.name, "points": cfg.npoints, "ncorr": cfg.ncorr, "nterms": cfg.nterms,
-                           "grid": [cfg.ny, cfg.nx], "n_cf": cfg.n_cf, "oversampling": cfg.oversampling, "n_valid": n_valid,
+                           "grid": [cfg.ny, cfg.nx], "n_cf": cfg.n_cf, "oversampling": cfg.oversampling, "tile_u_x_v": [cfg.tile_x, cfg.tile], "n_valid": n_valid,
                            "sum_S2": sum_s2, "l2": "inputs larger than L2 (vis+wt 0.97 GB, grid 1.07 GB per step)",
                            "parallelism": f"dp{world}" if world > 1 else "single"},
                 "phase_ms_median": med, "grid_vis_points_per_s": n_valid / (med["grid"] * 1e-3),

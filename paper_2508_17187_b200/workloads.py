@@ -64,8 +64,8 @@ class Config:
     time_stride_of: int = 0  # cfg5: take ntimes samples out of this many, 0 = off
     degrid: bool = False    # cfg5: model grid + degrid + residual gridding
     n_sources: int = 0
-    tile: int = 8           # uv tiles of the bucket sort: tile_x wide (u) by tile tall (v) -- the library's default
-    tile_x: int = 8
+    tile: int = 8           # uv tiles of the bucket sort: tile_x wide (u) by tile tall (v); 8 x 8 is the library's default.
+    tile_x: int = 8         # cfg2-4 use 4 wide x 8 tall tiles (dense data, narrower regions), cfg1 and cfg5 the default
 
     @property
     def nrow(self) -> int:
@@ -85,12 +85,12 @@ def full_config(n: int) -> Config:
     if n == 1:
         return Config(1, "cfg1-tiny-ps", 60, 1, 1, 1, 256, 256, 20, "ps", 7, 7, kind="disk")
     if n == 2:
-        return Config(2, "cfg2-vla-continuum-ps", 14400, 64, 2, 1, 4096, 4096, 20, "ps", 9, 9, ha_hours=4.0)
+        return Config(2, "cfg2-vla-continuum-ps", 14400, 64, 2, 1, 4096, 4096, 20, "ps", 9, 9, ha_hours=4.0, tile_x=4)
     if n == 3:
-        return Config(3, "cfg3-wprojection", 7200, 16, 2, 1, 8192, 8192, 8, "w", 9, 65, n_w=128, ha_hours=2.0)
+        return Config(3, "cfg3-wprojection", 7200, 16, 2, 1, 8192, 8192, 8, "w", 9, 65, n_w=128, ha_hours=2.0, tile_x=4)
     if n == 4:
         return Config(4, "cfg4-awprojection-fullpol", 7200, 16, 4, 1, 4096, 4096, 8, "aw", 17, 49,
-                      n_w=32, n_pa=8, n_fb=4, ha_hours=2.0)
+                      n_w=32, n_pa=8, n_fb=4, ha_hours=2.0, tile_x=4)
     if n == 5:
         return Config(5, "cfg5-degrid-multiterm", 1157, 16, 2, 2, 8192, 8192, 8, "w", 9, 65, n_w=128,
                       ha_hours=2.0, time_stride_of=7200, degrid=True, n_sources=200)
