@@ -154,18 +154,23 @@ __global__ void __launch_bounds__((lra_cw(NW) + 1) * 32) __maxnreg__(LRA_MAXNREG
     // Two releases per slot: its taps and records once this warp has loaded the last of them (the producer may then start
     // the copies of the slot's next batch), its results at the end of the batch.
     if (first >= count) lra_mbar_arrive(empty0 + 8 * slot);
+    const uint32_t bar_taps = empty0 + 8 * slot;
     for (unsigned q0 = first; q0 < count; q0 += 4 * PS) {   // this warp's points q0, q0 + PS, q0 + 2 PS, q0 + 3 PS
       float v[V];
 #pragma unroll
       for (int i = 0; i < V; ++i) v[i] = 0.f;
+      // index in this group of the warp's last point of the batch (>= 4: a later group).  One comparison per point against it
+      // is the cheaper form of the two tail conditions for one or two grids (cfg3 degridder 26.88 -> 26.67 ms); with three or
+      // four grids the plain conditions are (cfg4 44.88 -> 43.98 ms)
+      const unsigned last_u = (count - 1u - q0) / PS;
 #pragma unroll
       for (int u = 0; u < 4; ++u) {
         rec += 16 * PS;
         pc = *reinterpret_cast<const uint4*>(rec);
-        const uint32_t addr_next = lane_base + pc.x, mask_next = q0 + (u + 1) * PS < count ? lra_point_mask<NW>(pc.z, pc.w, pwarp) : 0u;
+        const uint32_t addr_next = lane_base + pc.x, mask_next = (NG <= 2 ? (unsigned)u < last_u : q0 + (u + 1) * PS < count) ? lra_point_mask<NW>(pc.z, pc.w, pwarp) : 0u;
         // the warp's last point of the batch: its taps were loaded during the point before (the arrival is ordered
         // after those loads), nothing of the slot but the result area is touched from here on
-        if (q0 + u * PS < count && q0 + (u + 1) * PS >= count) lra_mbar_arrive(empty0 + 8 * slot);
+        lra_mbar_arrive_if(bar_taps, NG <= 2 ? last_u == (unsigned)u : (q0 + u * PS < count && q0 + (u + 1) * PS >= count));
         lra_u64 P1[NG], P2[NG];
 #pragma unroll
         for (int g = 0; g < NG; ++g) P1[g] = P2[g] = 0ull;

@@ -180,6 +180,10 @@ __device__ __forceinline__ void lra_mbar_init(uint32_t bar, uint32_t count) {
 __device__ __forceinline__ void lra_mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
+// The arrival under a (warp-uniform) condition, as a branch around it: the address arithmetic of the barrier is skipped too
+__device__ __forceinline__ void lra_mbar_arrive_if(uint32_t bar, uint32_t cond) {
+  asm volatile("{\n.reg .pred p;\nsetp.eq.u32 p, %1, 0;\n@p bra.uni NOARR_%=;\nmbarrier.arrive.shared::cta.b64 _, [%0];\nNOARR_%=:\n}" ::"r"(bar), "r"(cond) : "memory");
+}
 // Adds to the transaction count only: the phase still needs the arrival (lra_mbar_arrive), which may come later.
 __device__ __forceinline__ void lra_mbar_expect_tx(uint32_t bar, uint32_t bytes) {
   asm volatile("mbarrier.expect_tx.relaxed.cta.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
