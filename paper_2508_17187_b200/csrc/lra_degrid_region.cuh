@@ -127,6 +127,26 @@ __global__ void __launch_bounds__((lra_cw(NW) + 1) * 32) __maxnreg__(LRA_MAXNREG
       const int ty = (int)(h.w / (unsigned)a.ntx), tx = (int)(h.w - (unsigned)ty * a.ntx);
       const int x0 = tx * a.tile_x - hh, y0 = ty * a.tile_y - hh;
       const unsigned magic = 0xffffffffu / (unsigned)a.rx + 1u;
+      if (NG <= 2 && x0 >= 0 && y0 >= 0 && x0 + a.rx <= a.nx && y0 + a.ry <= a.ny) {
+        // the region lies inside the grid (all tiles but those along its edges): no per-pixel bounds tests, one address per pixel
+        // (one or two grids; with four the second code path costs more than it saves: cfg4 43.95 -> 44.33 ms)
+        const float2* const g00 = a.grid + ((ptrdiff_t)y0 * a.nx + x0);
+        const unsigned npix = (unsigned)(a.rx * a.ry);
+#pragma unroll
+        for (int s = 0; s < KS; ++s) {
+#pragma unroll
+          for (int half = 0; half < 2; ++half) {
+            const unsigned e = 64u * (NW * s + pwarp) + 32u * half + lane;
+            const int y = (int)__umulhi(e, magic), x = (int)e - y * a.rx;
+            const float2* const px = g00 + (y * a.nx + x);
+#pragma unroll
+            for (int g = 0; g < NG; ++g) {
+              const float2 v = e < npix ? px[(size_t)g * a.plane] : make_float2(0.f, 0.f);
+              G[s][half][g] = lra_pack2(v.x, v.y);
+            }
+          }
+        }
+      } else
 #pragma unroll
       for (int s = 0; s < KS; ++s) {
 #pragma unroll

@@ -210,6 +210,14 @@ __device__ __forceinline__ void lra_tma_load_1d(uint32_t smem_dst, const void* g
 __device__ __forceinline__ void lra_red_add_v2(float2* addr, float re, float im) {
   asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(addr), "f"(re), "f"(im) : "memory");
 }
+// The same under a predicate formed inside the statement (no divergent branch around the reduction): pixel e belongs to the
+// region (e < npix) and the value is not +-0.
+__device__ __forceinline__ void lra_red_add_v2_nz(float2* addr, lra_u64 v, uint32_t e, uint32_t npix) {
+  asm volatile(
+      "{\n.reg .pred p, q;\n.reg .b32 lo, hi, t;\nmov.b64 {lo, hi}, %1;\nor.b32 t, lo, hi;\nshl.b32 t, t, 1;\n"
+      "setp.lt.u32 q, %2, %3;\nsetp.ne.and.u32 p, t, 0, q;\n@p red.global.add.v2.f32 [%0], {lo, hi};\n}"
+      ::"l"(addr), "l"(v), "r"(e), "r"(npix) : "memory");
+}
 // Packed fp32x2: d = a * b + c on both halves, one issue slot for two FMAs (FFMA2 on sm_100a).
 __device__ __forceinline__ lra_u64 lra_fma2(lra_u64 a, lra_u64 b, lra_u64 c) {
   lra_u64 d;
